@@ -1,0 +1,577 @@
+"""Pins for the CPU oracle (oracle/hough_oracle.c) -- CPU only, no CUDA.
+
+The paper prints no worked numeric example, so the oracle is pinned to what the
+mathematics fixes: explicit circle geometry (P1, P2), an independent fp64 vote count (P3), a division-free
+brute-force circle-membership test over all cells (P4), algebraic invariants (P5), definitional brute force
+and special cases for the peak finder (P6-P8), closed forms for track parameters (P9), an O(T^2) Python
+restatement and special cases for the cone clustering (P10, P11) and a hand-built end-to-end event (P12).
+None of these re-types the oracle's own fp32 operation sequence.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import hough_oracle as O
+from paper_1309_6275_b200 import workloads as W
+
+KMAX = 0.3e-3 * 3.8
+TWO_PI = 2.0 * math.pi
+
+
+# ----------------------------------------------------------------------------------------------
+# helpers (independent fp64 geometry)
+# ----------------------------------------------------------------------------------------------
+
+def circle_points(d0, phi0, kappa, arc_lengths):
+    """Points on the circle of signed curvature kappa that touches P = d0*(sin phi0, -cos phi0) with
+    tangent (cos phi0, sin phi0) there (reading R1), at signed arc lengths L from P."""
+    px, py = d0 * math.sin(phi0), -d0 * math.cos(phi0)
+    cx, cy = px - math.sin(phi0) / kappa, py + math.cos(phi0) / kappa        # C = P + n/kappa
+    th = phi0 + kappa * np.asarray(arc_lengths, dtype=np.float64)
+    x = cx + np.sin(th) / kappa
+    y = cy - np.cos(th) / kappa
+    # sanity: the points really are at distance 1/|kappa| from C and L = 0 is P
+    assert np.allclose(np.hypot(x - cx, y - cy), 1.0 / abs(kappa), rtol=1e-12)
+    return np.hypot(x, y), np.mod(np.arctan2(y, x), TWO_PI)
+
+
+def bin_centres(g: O.Grid):
+    dphi = TWO_PI / g.n_phi0
+    phi0c = (np.arange(g.n_phi0) + 0.5) * dphi
+    dk = 2.0 * float(np.float32(g.kappa_max)) / g.n_kappa
+    kc = -float(np.float32(g.kappa_max)) + (np.arange(g.n_kappa) + 0.5) * dk
+    if g.n_d0 > 1:
+        d0c = (np.float32(g.d0_min).astype(np.float64)
+               + (np.arange(g.n_d0) + 0.5) * ((float(np.float32(g.d0_max)) - float(np.float32(g.d0_min))) / g.n_d0))
+        d0c = d0c.astype(np.float32).astype(np.float64)
+    else:
+        d0c = np.zeros(1)
+    return d0c, phi0c, kc, dk
+
+
+def u_double(g: O.Grid, r, phi, d0, phi0):
+    """kappa-bin coordinate of hit (r, phi) in column (d0, phi0), all in fp64, north_star's formula."""
+    s = np.sin(phi - phi0)
+    kap = 2.0 * (r * s + d0) / (r * r + 2.0 * d0 * r * s + d0 * d0)
+    kmax = float(np.float32(g.kappa_max))
+    return (kap + kmax) * (g.n_kappa / (2.0 * kmax))
+
+
+# ----------------------------------------------------------------------------------------------
+# O-0 tables
+# ----------------------------------------------------------------------------------------------
+
+def test_tables_are_bin_centres():
+    g = O.Grid(64, 32, 8, KMAX, -50.0, 50.0)
+    c0, s0, d0c, inv_dk = O.tables(g)
+    d0_ref, phi0c, _, dk = bin_centres(g)
+    assert np.allclose(c0, np.cos(phi0c), atol=1e-7) and np.allclose(s0, np.sin(phi0c), atol=1e-7)
+    assert np.allclose(c0.astype(np.float64) ** 2 + s0.astype(np.float64) ** 2, 1.0, atol=3e-7)
+    assert np.array_equal(d0c.astype(np.float64), d0_ref)
+    assert np.allclose(d0c, -50.0 + (np.arange(8) + 0.5) * 12.5)
+    assert d0c[0] == -d0c[-1]                                   # symmetric grid
+    assert abs(float(inv_dk) * dk - 1.0) < 1e-6
+
+
+# ----------------------------------------------------------------------------------------------
+# P1 / P2: explicit circle geometry -> generating bin (prompt 2D and displaced 3D), mirror solution
+# ----------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mode", ["2d", "3d"])
+def test_P1_circle_points_vote_into_generating_kappa_bin(mode):
+    rng = np.random.default_rng(11)
+    g = O.Grid(128, 64, 1, KMAX) if mode == "2d" else O.Grid(128, 64, 16, KMAX, -50.0, 50.0)
+    d0c, phi0c, kc, dk = bin_centres(g)
+    kmax = float(np.float32(g.kappa_max))
+    checked = 0
+    for _ in range(300):
+        idx_d = int(rng.integers(g.n_d0)); ip = int(rng.integers(g.n_phi0))
+        kappa = rng.uniform(-0.98, 0.98) * kmax
+        if abs(kappa) < 1e-6:
+            continue
+        d0, phi0 = float(d0c[idx_d]), float(phi0c[ip])
+        # forward quarter turn only, and stay inside a 1.1 m tracker
+        L = rng.uniform(0.02, 0.9, 12) * min(0.5 * math.pi / abs(kappa), 1000.0)
+        r, phi = circle_points(d0, phi0, kappa, L)
+        keep = (r > 25.0) & (r < 1100.0)
+        r, phi = r[keep], phi[keep]
+        if r.size == 0:
+            continue
+        u_true = (kappa + kmax) / dk
+        if abs(u_true - round(u_true)) < 0.02:                  # too close to a bin edge for fp32 inputs
+            continue
+        ik_true = int(math.floor(u_true))
+        layer = (np.arange(r.size) % 8).astype(np.uint8)
+        cnt, msk, votes = O.vote_columns(g, r.astype(np.float32), phi.astype(np.float32), layer, [idx_d], [ip])
+        assert votes == r.size, (mode, d0, phi0, kappa, r, phi)
+        assert cnt[0, ik_true] == r.size and cnt[0].sum() == r.size
+        want_mask = 0
+        for l in layer:
+            want_mask |= 1 << int(l)
+        assert msk[0, ik_true] == want_mask
+        # R5 mirror: same circle traversed backwards = (-d0, phi0 + pi, -kappa)
+        if g.n_phi0 % 2 == 0 and (g.n_d0 == 1 or g.d0_min == -g.d0_max):
+            idm, ipm, ikm = g.n_d0 - 1 - idx_d, (ip + g.n_phi0 // 2) % g.n_phi0, g.n_kappa - 1 - ik_true
+            cm, mm, vm = O.vote_columns(g, r.astype(np.float32), phi.astype(np.float32), layer, [idm], [ipm])
+            assert cm[0, ikm] == r.size and vm == r.size
+        checked += 1
+    assert checked > 150
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_P2_noiseless_bin_centred_track_peaks_at_generating_bin(cfg):
+    """north_star check 1: a noiseless single track peaks at its generating bin with count = number of
+    layers it crosses (a feature with N contributing inputs collects N votes)."""
+    w = W.config(cfg)
+    g = O.Grid.from_workload(w)
+    d0c, phi0c, kc, dk = bin_centres(g)
+    radii = np.asarray(w.radii)
+    rng = np.random.default_rng(5 + cfg)
+    for _ in range(4):
+        idx_d = int(rng.integers(g.n_d0)); ip = int(rng.integers(g.n_phi0)); ik = int(rng.integers(8, g.n_kappa - 8))
+        d0, phi0, kappa = float(d0c[idx_d]), float(phi0c[ip]), float(kc[ik])
+        # layer crossings of this circle, forward from P, by dense arc sampling + bisection (no formula inversion)
+        Ls = np.linspace(0.0, min(math.pi / abs(kappa), 4000.0), 200001)
+        rr, _ = circle_points(d0, phi0, kappa, Ls)
+        hits_r, hits_phi, hits_l = [], [], []
+        for l, R in enumerate(radii):
+            sgn = np.sign(rr - R)
+            cross = np.nonzero(sgn[:-1] * sgn[1:] < 0)[0]
+            if cross.size == 0:
+                continue
+            lo, hi = Ls[cross[0]], Ls[cross[0] + 1]
+            for _ in range(60):
+                mid = 0.5 * (lo + hi)
+                rm, _ = circle_points(d0, phi0, kappa, [mid])
+                if (rm[0] - R) * (circle_points(d0, phi0, kappa, [lo])[0][0] - R) <= 0:
+                    hi = mid
+                else:
+                    lo = mid
+            rm, pm = circle_points(d0, phi0, kappa, [0.5 * (lo + hi)])
+            hits_r.append(R); hits_phi.append(pm[0]); hits_l.append(l)
+        n_cross = len(hits_r)
+        assert n_cross >= (len(radii) - 2 if cfg == 1 else 1)
+        if cfg == 1:
+            assert n_cross == len(radii)                         # prompt track crosses every layer
+        cnt, msk, _ = O.vote(g, np.float32(hits_r), np.float32(hits_phi), np.uint8(hits_l),
+                             id_range=(max(idx_d - 1, 0), min(idx_d + 2, g.n_d0)))
+        assert cnt[idx_d, ip, ik] == n_cross
+        assert bin(int(msk[idx_d, ip, ik])).count("1") == n_cross
+        if n_cross >= 2:
+            pk, tot = O.peaks(g, cnt, msk, n_cross, 64)
+            assert (idx_d * g.n_phi0 + ip) * g.n_kappa + ik in pk["lin"].tolist()
+            assert cnt.max() == n_cross
+
+
+def test_P2_dropping_hits_lowers_the_peak_by_exactly_that_many():
+    """Hough is tolerant to missing hits: each dropped hit removes exactly one vote / one layer."""
+    w = W.config(1); g = O.Grid.from_workload(w)
+    d0c, phi0c, kc, dk = bin_centres(g)
+    ip, ik = 77, 40
+    radii = np.asarray(w.radii)
+    phi = phi0c[ip] + np.arcsin(kc[ik] * radii / 2.0)            # prompt closed form (R26)
+    for drop in range(0, 4):
+        keep = np.arange(radii.size) >= drop
+        cnt, msk, _ = O.vote(g, radii[keep].astype(np.float32), np.mod(phi[keep], TWO_PI).astype(np.float32),
+                             np.arange(radii.size, dtype=np.uint8)[keep])
+        assert cnt[0, ip, ik] == radii.size - drop
+        assert int(msk[0, ip, ik]) == (0xFF >> drop) << drop
+        for l_min in (radii.size - drop, radii.size - drop + 1):
+            pk, _ = O.peaks(g, cnt, msk, l_min, 64)
+            assert ((ip * g.n_kappa + ik) in pk["lin"].tolist()) == (l_min <= radii.size - drop)
+
+
+# ----------------------------------------------------------------------------------------------
+# P3: conservation -- total votes = number of in-range (hit, d0, phi0) triples (independent fp64 count)
+# ----------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("cfg,nd,nphi,nk", [(1, 1, 512, 256), (2, 8, 128, 64), (4, 16, 64, 32)])
+def test_P3_total_votes_equal_in_range_triples(cfg, nd, nphi, nk):
+    w = W.scaled(W.config(cfg), n_d0=nd, n_phi0=nphi, n_kappa=nk)
+    g = O.Grid.from_workload(w)
+    r, phi, layer, _ = W.generate_event(w, 0)
+    cnt, msk, votes = O.vote(g, r, phi, layer)
+    assert votes == int(cnt.astype(np.int64).sum())
+    d0c, phi0c, _, _ = bin_centres(g)
+    R = r.astype(np.float64)[:, None, None]; PH = phi.astype(np.float64)[:, None, None]
+    u = u_double(g, R, PH, d0c[None, :, None], phi0c[None, None, :])
+    inside = (u >= 0) & (u < g.n_kappa)
+    ambiguous = (np.abs(u) < 2e-3) | (np.abs(u - g.n_kappa) < 2e-3)
+    assert abs(votes - int(inside.sum())) <= int(ambiguous.sum())
+    # per-layer: votes carrying layer l = in-range triples of layer-l hits
+    for l in range(w.n_layers):
+        sel = layer == l
+        c_l, _, v_l = O.vote(g, r[sel], phi[sel], layer[sel])
+        assert abs(v_l - int(inside[sel].sum())) <= int(ambiguous[sel].sum())
+        assert np.all((msk[c_l > 0] >> l) & 1)
+
+
+def test_P3_closed_form_single_hit_2d():
+    g = O.Grid(1024, 512, 1, KMAX)
+    for rr in (40.0, 250.0, 600.0, 1000.0):
+        for ph in (0.1, 3.0, 6.2):
+            _, _, votes = O.vote(g, np.float32([rr]), np.float32([ph]), np.uint8([0]))
+            expect = g.n_phi0 * (2.0 / math.pi) * math.asin(KMAX * rr / 2.0)
+            assert abs(votes - expect) <= 4, (rr, ph, votes, expect)
+
+
+# ----------------------------------------------------------------------------------------------
+# P4: brute-force, division-free circle membership over ALL cells x ALL hits
+# ----------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("nd,nphi,nk,dmax", [(1, 64, 64, 0.0), (8, 32, 32, 50.0), (16, 32, 16, 100.0)])
+def test_P4_bruteforce_circle_fit_matches(nd, nphi, nk, dmax):
+    """Hit x lies in cell (id, ip, ik) iff F(k_lo) <= 0 < F(k_hi), F(k) = (k/2)|x-P|^2 - (x-P).n  (fp64,
+    Cartesian, no division, no sine-difference identity)."""
+    base = W.config(2 if nd > 1 else 1)
+    w = W.scaled(base, n_d0=nd, n_phi0=nphi, n_kappa=nk, d0_min=-dmax, d0_max=dmax, n_noise=(150, 150))
+    g = O.Grid.from_workload(w)
+    r, phi, layer, _ = W.generate_event(w, 3)
+    cnt, msk, _ = O.vote(g, r, phi, layer)
+    d0c, phi0c, kc, dk = bin_centres(g)
+    x = r.astype(np.float64) * np.cos(phi.astype(np.float64))
+    y = r.astype(np.float64) * np.sin(phi.astype(np.float64))
+    kmax = float(np.float32(g.kappa_max))
+    k_edges = -kmax + np.arange(nk + 1) * dk
+    brute = np.zeros(g.shape, np.int64)
+    brute_mask = np.zeros(g.shape, np.int64)
+    near_edge = np.zeros(g.shape, bool)
+    for i_d in range(nd):
+        for ip in range(nphi):
+            px, py = d0c[i_d] * math.sin(phi0c[ip]), -d0c[i_d] * math.cos(phi0c[ip])
+            nx, ny = -math.sin(phi0c[ip]), math.cos(phi0c[ip])
+            q2 = (x - px) ** 2 + (y - py) ** 2
+            dn = (x - px) * nx + (y - py) * ny
+            F = 0.5 * k_edges[None, :] * q2[:, None] - dn[:, None]                # [H, NK+1]
+            inside = (F[:, :-1] <= 0) & (F[:, 1:] > 0)
+            brute[i_d, ip] = inside.sum(0)
+            for l in range(w.n_layers):
+                brute_mask[i_d, ip] |= (inside[layer == l].any(0).astype(np.int64) << l)
+            # candidates whose fp64 bin coordinate is within 2e-3 of an integer may round either way in fp32
+            u = u_double(g, r.astype(np.float64), phi.astype(np.float64), d0c[i_d], phi0c[ip])
+            amb = np.abs(u - np.round(u)) < 2e-3
+            for uu in u[amb]:
+                for b in (int(math.floor(uu)), int(math.floor(uu)) - 1, int(math.floor(uu)) + 1):
+                    if 0 <= b < nk:
+                        near_edge[i_d, ip, b] = True
+    diff = (cnt.astype(np.int64) != brute) | (msk.astype(np.int64) != brute_mask)
+    assert brute.sum() > 0.05 * r.size * nd * nphi               # the test is not vacuous
+    assert not np.any(diff & ~near_edge), np.argwhere(diff & ~near_edge)[:10]
+    assert diff.sum() <= max(8, 2e-4 * brute.sum())
+
+
+# ----------------------------------------------------------------------------------------------
+# P5: invariants of the vote
+# ----------------------------------------------------------------------------------------------
+
+def test_P5_vote_invariants():
+    w = W.scaled(W.config(2), n_d0=8, n_phi0=128, n_kappa=64)
+    g = O.Grid.from_workload(w)
+    r, phi, layer, _ = W.generate_event(w, 1)
+    cnt, msk, votes = O.vote(g, r, phi, layer)
+    pc = np.vectorize(lambda m: bin(int(m)).count("1"))(msk)
+    assert np.array_equal(msk == 0, cnt == 0)
+    assert np.all(cnt >= pc)
+    assert np.all(cnt.astype(np.int64).sum(axis=2) <= r.size)    # one vote per (hit, column) at most
+    # additivity / OR over a split of the hits, and permutation invariance (R25)
+    h = r.size // 3
+    ca, ma, _ = O.vote(g, r[:h], phi[:h], layer[:h]); cb, mb, _ = O.vote(g, r[h:], phi[h:], layer[h:])
+    assert np.array_equal(cnt, ca + cb) and np.array_equal(msk, ma | mb)
+    perm = np.random.default_rng(0).permutation(r.size)
+    cp_, mp_, _ = O.vote(g, r[perm], phi[perm], layer[perm])
+    assert np.array_equal(cnt, cp_) and np.array_equal(msk, mp_)
+    # R9 invalid layers are ignored entirely
+    bad = layer.copy(); bad[::5] = 200
+    cbad, mbad, _ = O.vote(g, r, phi, bad)
+    keep = bad < w.n_layers
+    ck, mk, _ = O.vote(g, r[keep], phi[keep], layer[keep])
+    assert np.array_equal(cbad, ck) and np.array_equal(mbad, mk)
+    # restricted ranges and sampled columns agree with the full vote
+    csub, msub, _ = O.vote(g, r, phi, layer, id_range=(2, 5), ip_range=(10, 40))
+    assert np.array_equal(csub[2:5, 10:40], cnt[2:5, 10:40]) and csub.sum() == cnt[2:5, 10:40].sum()
+    cc, mc, _ = O.vote_columns(g, r, phi, layer, [0, 7, 3], [5, 127, 64])
+    assert np.array_equal(cc[1], cnt[7, 127]) and np.array_equal(mc[2], msk[3, 64]) and np.array_equal(cc[0], cnt[0, 5])
+
+
+def test_P5_degenerate_inputs_vote_nowhere():
+    g = O.Grid(64, 32, 4, KMAX, -50.0, 50.0)
+    for rr, ph in [(np.nan, 1.0), (100.0, np.nan), (np.inf, 1.0), (100.0, np.inf), (0.0, 1.0)]:
+        cnt, msk, votes = O.vote(g, np.float32([rr]), np.float32([ph]), np.uint8([0]))
+        if rr == 0.0:
+            # r = 0: kappa = 2 d0 / d0^2 = 2/d0 -- far outside |kappa| <= kmax for |d0| >= 6 mm
+            assert votes == 0
+        else:
+            assert votes == 0 and cnt.sum() == 0 and msk.sum() == 0
+
+
+# ----------------------------------------------------------------------------------------------
+# P6-P8: peak finder
+# ----------------------------------------------------------------------------------------------
+
+def brute_peaks(cnt, msk, l_min):
+    """Definition of O-3 written with explicit neighbour loops in Python (tiny grids only)."""
+    ND, NP, NK = cnt.shape
+    out = []
+    for i_d in range(ND):
+        for ip in range(NP):
+            for ik in range(NK):
+                if bin(int(msk[i_d, ip, ik])).count("1") < l_min:
+                    continue
+                lin = (i_d * NP + ip) * NK + ik
+                c = int(cnt[i_d, ip, ik]); ok = True
+                for dd in (-1, 0, 1):
+                    for dp in (-1, 0, 1):
+                        for dk_ in (-1, 0, 1):
+                            if dd == dp == dk_ == 0:
+                                continue
+                            j_d, jk = i_d + dd, ik + dk_
+                            if not (0 <= j_d < ND and 0 <= jk < NK):
+                                continue
+                            jp = (ip + dp) % NP
+                            nlin = (j_d * NP + jp) * NK + jk
+                            cn = int(cnt[j_d, jp, jk])
+                            if cn > c or (cn == c and nlin < lin):
+                                ok = False
+                if ok:
+                    out.append((lin, c, int(msk[i_d, ip, ik])))
+    return out
+
+
+@pytest.mark.parametrize("shape", [(1, 8, 8), (1, 16, 12), (3, 6, 10), (4, 8, 8), (2, 4, 4)])
+def test_P6_peaks_match_definition(shape):
+    rng = np.random.default_rng(sum(shape))
+    g = O.Grid(shape[1], shape[2], shape[0], KMAX, -10.0, 10.0)
+    for trial in range(6):
+        cnt = rng.integers(0, 4 if trial % 2 else 12, shape).astype(np.uint16)     # many ties
+        msk = np.where(cnt > 0, rng.integers(1, 256, shape), 0).astype(np.uint16)
+        for l_min in (1, 2, 4):
+            pk, tot = O.peaks(g, cnt, msk, l_min, 10000)
+            want = brute_peaks(cnt, msk, l_min)
+            assert tot == len(want)
+            assert [(int(p["lin"]), int(p["count"]), int(p["mask"])) for p in pk] == want
+            # truncation convention: true total, first max_peaks in index order
+            pk2, tot2 = O.peaks(g, cnt, msk, l_min, 2)
+            assert tot2 == tot and [int(p["lin"]) for p in pk2] == [x[0] for x in want[:2]]
+
+
+def test_P7_peak_special_cases():
+    g = O.Grid(8, 6, 3, KMAX, -10.0, 10.0)
+    z = np.zeros(g.shape, np.uint16)
+    assert O.peaks(g, z, z, 1, 16)[1] == 0
+    full = np.full(g.shape, 5, np.uint16); fm = np.full(g.shape, 0xFF, np.uint16)
+    pk, tot = O.peaks(g, full, fm, 8, 16)
+    assert tot == 1 and pk["lin"][0] == 0                       # plateau -> lowest linear index only
+    for (i_d, ip, ik) in [(0, 0, 0), (2, 7, 5), (1, 0, 3), (1, 7, 0), (0, 3, 5)]:   # seam and borders
+        c = z.copy(); m = z.copy(); c[i_d, ip, ik] = 3; m[i_d, ip, ik] = 0b111
+        pk, tot = O.peaks(g, c, m, 3, 16)
+        assert tot == 1 and pk["lin"][0] == (i_d * 8 + ip) * 6 + ik and pk["count"][0] == 3 and pk["mask"][0] == 7
+        assert O.peaks(g, c, m, 4, 16)[1] == 0
+    # two equal adjacent bins across the phi0 seam: ip = 7 and ip = 0 are neighbours, lower lin (ip = 0) wins
+    c = z.copy(); m = z.copy()
+    c[1, 7, 2] = c[1, 0, 2] = 4; m[1, 7, 2] = m[1, 0, 2] = 0xF
+    pk, tot = O.peaks(g, c, m, 4, 16)
+    assert tot == 1 and pk["lin"][0] == (1 * 8 + 0) * 6 + 2
+    # R13: a neighbour that fails L_min still suppresses
+    c = z.copy(); m = z.copy(); c[0, 2, 2] = 5; m[0, 2, 2] = 0b1; c[0, 2, 3] = 4; m[0, 2, 3] = 0xF
+    assert O.peaks(g, c, m, 4, 16)[1] == 0
+
+
+def test_P8_peak_invariants_on_a_real_accumulator():
+    w = W.scaled(W.config(2), n_d0=8, n_phi0=128, n_kappa=64)
+    g = O.Grid.from_workload(w)
+    r, phi, layer, _ = W.generate_event(w, 0)
+    cnt, msk, _ = O.vote(g, r, phi, layer)
+    prev = None
+    for l_min in (1, 2, 3, 4, 6):
+        pk, tot = O.peaks(g, cnt, msk, l_min, 1 << 20)
+        lin = pk["lin"].astype(np.int64)
+        assert tot == lin.size and np.all(np.diff(lin) > 0)
+        assert all(bin(int(m)).count("1") >= l_min for m in pk["mask"])
+        i_d, ip, ik = lin // (128 * 64), (lin // 64) % 128, lin % 64
+        coords = set(zip(i_d.tolist(), ip.tolist(), ik.tolist()))
+        for (a, b, c) in coords:                                # no two peaks are neighbours, seam included
+            for dd in (-1, 0, 1):
+                for dp in (-1, 0, 1):
+                    for dk_ in (-1, 0, 1):
+                        if dd == dp == dk_ == 0:
+                            continue
+                        assert (a + dd, (b + dp) % 128, c + dk_) not in coords
+        if prev is not None:
+            assert set(lin.tolist()) <= prev                    # raising L_min only removes peaks
+        prev = set(lin.tolist())
+    assert tot >= 0
+
+
+# ----------------------------------------------------------------------------------------------
+# P9: tracks
+# ----------------------------------------------------------------------------------------------
+
+def test_P9_track_closed_forms():
+    g = O.Grid(64, 32, 8, KMAX, -50.0, 50.0, b_tesla=3.8)
+    d0c, phi0c, kc, dk = bin_centres(g)
+    lins = [(i_d * 64 + ip) * 32 + ik for i_d in (0, 3, 7) for ip in (0, 31, 63) for ik in (0, 5, 15, 16, 26, 31)]
+    pk = np.zeros(len(lins), O.PEAK_DTYPE); pk["lin"] = lins
+    t = O.tracks(g, pk)
+    for j, lin in enumerate(lins):
+        i_d, ip, ik = lin // (64 * 32), (lin // 32) % 64, lin % 32
+        assert abs(t["pt"][j] * abs(kc[ik]) / (0.3e-3 * 3.8) - 1) < 1e-6
+        assert abs(t["phi0"][j] - phi0c[ip]) < 1e-6 and t["d0"][j] == np.float32(d0c[i_d])
+        assert t["q"][j] == (1 if kc[ik] < 0 else -1) and t["jet"][j] == -1
+        # mirror bin: same pT, opposite charge
+        jm = lins.index((i_d * 64 + ip) * 32 + (31 - ik)) if (i_d * 64 + ip) * 32 + (31 - ik) in lins else None
+        if jm is not None:
+            assert t["pt"][jm] == t["pt"][j] and t["q"][jm] == -t["q"][j]
+    # a 1 GeV track sits at |kappa| = kmax: outermost bins are just above 1 GeV
+    assert 1.0 < t["pt"][lins.index(0)] < 1.04
+    # 2D mode: d0 = 0
+    g2 = O.Grid(64, 32, 1, KMAX)
+    pk2 = np.zeros(1, O.PEAK_DTYPE); pk2["lin"] = [5 * 32 + 3]
+    assert O.tracks(g2, pk2)["d0"][0] == 0.0
+
+
+# ----------------------------------------------------------------------------------------------
+# P10 / P11: jets
+# ----------------------------------------------------------------------------------------------
+
+def brute_jets(g, pk, cone_rad, d0_cut, n_min):
+    NP, NK = g.n_phi0, g.n_kappa
+    d0c, phi0c, kc, _ = bin_centres(g)
+    lin = pk["lin"].astype(np.int64)
+    ik, ip, i_d = lin % NK, (lin // NK) % NP, lin // (NK * NP)
+    cone_bins = int(math.floor(float(np.float32(cone_rad)) * NP / TWO_PI))
+    key = [(abs(2 * int(k) - (NK - 1)), j) for j, k in enumerate(ik)]
+    disp = [(g.n_d0 > 1) and (abs(np.float32(d0c[d])) > np.float32(d0_cut)) for d in i_d]
+    un = set(range(lin.size)); jets = []; assign = [-1] * lin.size
+    while un:
+        seed = min(un, key=lambda j: key[j])
+        mem = sorted(m for m in un if min(abs(ip[m] - ip[seed]), NP - abs(ip[m] - ip[seed])) <= cone_bins)
+        for m in mem:
+            assign[m] = len(jets)
+        un -= set(mem)
+        jets.append((seed, len(mem), sum(disp[m] for m in mem), mem))
+    flag = int(any(j[2] >= n_min for j in jets))
+    return jets, assign, flag
+
+
+@pytest.mark.parametrize("nd", [1, 8])
+def test_P10_jets_match_bruteforce_and_invariants(nd):
+    g = O.Grid(128, 64, nd, KMAX, -20.0, 20.0)
+    rng = np.random.default_rng(100 + nd)
+    for trial in range(20):
+        T = int(rng.integers(1, 33))
+        lin = np.sort(rng.choice(g.n_d0 * g.n_phi0 * g.n_kappa, T, replace=False))
+        if trial % 3 == 0:                                      # cluster them in phi0 so jets have many members
+            ip = (rng.integers(0, 128) + rng.integers(-6, 7, T)) % 128
+            lin = np.sort(np.unique((rng.integers(0, nd, T) * 128 + ip) * 64 + rng.integers(0, 64, T)))
+            T = lin.size
+        pk = np.zeros(T, O.PEAK_DTYPE); pk["lin"] = lin
+        cone = float(rng.choice([0.0, 0.05, 0.2, 0.4, 1.0]))
+        trk, jets, n_jets, flag = O.jets(g, pk, cone, 2.0, 3, 64)
+        bj, assign, bflag = brute_jets(g, pk, cone, 2.0, 3)
+        assert n_jets == len(bj) and flag == bflag
+        assert trk["jet"].tolist() == assign
+        for J, (seed, n, nd_, mem) in enumerate(bj):
+            assert (jets["seed_track"][J], jets["n_tracks"][J], jets["n_displaced"][J]) == (seed, n, nd_)
+            assert abs(jets["sum_pt"][J] - trk["pt"][mem].astype(np.float64).sum()) <= 1e-5 * jets["sum_pt"][J]
+            assert jets["phi"][J] == trk["phi0"][seed]
+        assert jets["n_tracks"].sum() == T                      # every stored track in exactly one jet
+        assert set(trk["jet"].tolist()) == set(range(n_jets))
+        if nd == 1:
+            assert flag == 0 and jets["n_displaced"].sum() == 0  # IP tracks form an ordinary jet
+        # seeds in non-decreasing key order; later seeds outside every earlier seed's cone
+        ik = lin % 64; ip = (lin // 64) % 128
+        keys = [abs(2 * int(ik[s]) - 63) for s in jets["seed_track"]]
+        assert keys == sorted(keys)
+        cb = int(math.floor(float(np.float32(cone)) * 128 / TWO_PI))
+        seeds = jets["seed_track"].tolist()
+        for a in range(len(seeds)):
+            for b in range(a):
+                d = abs(int(ip[seeds[a]]) - int(ip[seeds[b]]))
+                assert min(d, 128 - d) > cb
+
+
+def test_P11_jet_special_cases():
+    g = O.Grid(128, 64, 8, KMAX, -20.0, 20.0)
+    empty = np.zeros(0, O.PEAK_DTYPE)
+    trk, jets, n, flag = O.jets(g, empty, 0.4, 2.0, 3, 8)
+    assert n == 0 and flag == 0 and jets.size == 0 and trk.size == 0
+    lin = np.sort(np.random.default_rng(3).choice(8 * 128 * 64, 40, replace=False))
+    pk = np.zeros(40, O.PEAK_DTYPE); pk["lin"] = lin
+    _, jets, n, _ = O.jets(g, pk, 3.2, 2.0, 3, 8)               # cone >= pi -> one jet
+    assert n == 1 and jets["n_tracks"][0] == 40
+    trk, jets, n, _ = O.jets(g, pk, 0.0, 2.0, 3, 64)            # cone_bins = 0 -> one jet per distinct ip
+    assert n == np.unique((lin // 64) % 128).size
+    # capacity: true total reported, only first max_jets stored, tracks of unstored jets keep jet = -1
+    trk2, jets2, n2, _ = O.jets(g, pk, 0.0, 2.0, 3, 5)
+    assert n2 == n and jets2.size == 5 and np.array_equal(jets2, jets[:5])
+    assert np.array_equal(trk2["jet"], np.where(trk["jet"] < 5, trk["jet"], -1))
+    # displaced rule R20: strict |d0c| > cut on bin centres (bins at +-2.5 mm: > 2 yes, > 2.5 no)
+    pk3 = np.zeros(3, O.PEAK_DTYPE); pk3["lin"] = [(3 * 128 + 10) * 64 + 5, (3 * 128 + 11) * 64 + 9, (4 * 128 + 12) * 64 + 30]
+    assert O.jets(g, pk3, 0.4, 2.0, 3, 8)[3] == 1 and O.jets(g, pk3, 0.4, 2.0, 3, 8)[1]["n_displaced"][0] == 3
+    assert O.jets(g, pk3, 0.4, 2.5, 3, 8)[3] == 0
+    assert O.jets(g, pk3, 0.4, 2.0, 4, 8)[3] == 0
+
+
+# ----------------------------------------------------------------------------------------------
+# P12: hand-built end-to-end event
+# ----------------------------------------------------------------------------------------------
+
+def _forward_hits_on_layers(d0, phi0, kappa, radii):
+    """First forward crossing of each layer, by bisection on explicit circle points."""
+    out = []
+    Ls = np.linspace(0.0, min(math.pi / abs(kappa), 4000.0), 100001)
+    rr, _ = circle_points(d0, phi0, kappa, Ls)
+    for l, R in enumerate(radii):
+        sgn = np.sign(rr - R)
+        cross = np.nonzero(sgn[:-1] * sgn[1:] < 0)[0]
+        if cross.size == 0:
+            continue
+        lo, hi = Ls[cross[0]], Ls[cross[0] + 1]
+        f_lo = circle_points(d0, phi0, kappa, [lo])[0][0] - R
+        for _ in range(60):
+            mid = 0.5 * (lo + hi)
+            f_mid = circle_points(d0, phi0, kappa, [mid])[0][0] - R
+            if f_mid * f_lo <= 0:
+                hi = mid
+            else:
+                lo, f_lo = mid, f_mid
+        _, pm = circle_points(d0, phi0, kappa, [0.5 * (lo + hi)])
+        out.append((l, R, pm[0]))
+    return out
+
+
+@pytest.mark.parametrize("k_disp", [2, 3, 4])
+def test_P12_hand_built_event_end_to_end(k_disp):
+    w = W.scaled(W.config(2), n_d0=16, n_phi0=256, n_kappa=128, d0_min=-40.0, d0_max=40.0)
+    g = O.Grid.from_workload(w)
+    d0c, phi0c, kc, dk = bin_centres(g)                          # d0 bins of 5 mm: centres +-2.5, +-7.5, ...
+    # k displaced tracks (|d0c| = 7.5 or 12.5 mm > 2 mm) inside one 0.4 rad cone (256 bins -> cone_bins = 16),
+    # 2 prompt-like tracks (|d0c| = 2.5 mm is NOT > 2.5... use cut 3 mm) far away in phi0.
+    disp_bins = [(9, 40, 100), (10, 44, 30), (5, 47, 90), (6, 36, 20)][:k_disp]
+    prompt_bins = [(8, 100, 70), (7, 103, 40)]
+    hits = []
+    for (i_d, ip, ik) in disp_bins + prompt_bins:
+        hits += _forward_hits_on_layers(float(d0c[i_d]), float(phi0c[ip]), float(kc[ik]), w.radii)
+    layer = np.uint8([h[0] for h in hits]); r = np.float32([h[1] for h in hits]); phi = np.float32([h[2] for h in hits])
+    res = O.run_event(g, r, phi, layer, l_min=8, max_peaks=256, max_jets=32, cone_rad=0.4, d0_cut_mm=3.0,
+                      n_displaced_min=3)
+    lin_of = lambda b: (b[0] * 256 + b[1]) * 128 + b[2]
+    mirror = lambda b: (15 - b[0], (b[1] + 128) % 256, 127 - b[2])
+    expect = sorted(lin_of(b) for b in disp_bins + prompt_bins) + []
+    expect = sorted(expect + [lin_of(mirror(b)) for b in disp_bins + prompt_bins])
+    assert res.n_peaks == len(expect) and res.peaks["lin"].tolist() == expect
+    # 8 own hits each; a stray hit of another track may share the bin (count >= popcount(mask), R11)
+    assert np.all(res.peaks["count"] >= 8) and np.all(res.peaks["count"] <= 9) and np.all(res.peaks["mask"] == 0xFF)
+    # jets: {displaced group}, {prompt group} and their two mirror images (R5) -> 4 jets
+    assert res.n_jets == 4
+    nd = sorted(res.jets["n_displaced"].tolist())
+    assert nd == [0, 0, k_disp, k_disp]
+    assert sorted(res.jets["n_tracks"].tolist()) == sorted([2, 2, k_disp, k_disp])
+    assert res.flag == (1 if k_disp >= 3 else 0)
+    # seed of each jet is its highest-pT member = smallest |2 ik - (NK-1)|
+    for J in range(4):
+        mem = np.nonzero(res.tracks["jet"] == J)[0]
+        a = np.abs(2 * (res.peaks["lin"][mem].astype(np.int64) % 128) - 127)
+        assert res.jets["seed_track"][J] == mem[np.argmin(a)]
+        assert abs(res.jets["sum_pt"][J] - res.tracks["pt"][mem].sum()) < 1e-4 * res.jets["sum_pt"][J]
