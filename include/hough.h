@@ -1,0 +1,167 @@
+/*
+ * hough.h -- C-ABI boundary of the B200-native Hough trigger hot path.
+ *
+ * Method: Halyo, LeGresley, Lujan, "Massively Parallel Computing and the Search for Jets and Black Holes
+ * at the LHC", arXiv:1309.6275 (text in PAPER.md).  The paper gives the pipeline in words only
+ * (section 6: "the hit data for an event is processed using the Hough transform to compute
+ * the parameter space representation.  Candidate tracks are identified by finding local maxima, or peaks,
+ * in the parameter space"); the concrete formulas, bin layout and selection rules are those of
+ * BASELINE.json:north_star as read in DESIGN.md ("Readings").
+ *
+ * Everything here is plain C: opaque context, POD structs, raw pointers.  Unless a parameter is marked
+ * HOST, every pointer is a DEVICE pointer owned (allocated and freed) by the caller; `stream` is a
+ * cudaStream_t passed as void*.  All work is enqueued on `stream`; only hough_create, hough_destroy,
+ * hough_status, hough_trigger_host and hough_microbench synchronise.  Calls on one context must be
+ * stream-ordered by the caller (the context owns a per-call workspace).  No entry point allocates or
+ * frees device memory except hough_create / hough_destroy.  There is no CPU fallback anywhere: without a
+ * CUDA device hough_create fails with HOUGH_ECUDA.
+ *
+ * Notation: E events; ND, NPHI, NK bins in d0, phi0, kappa; bin (id, ip, ik) has linear index
+ * lin = (id*NPHI + ip)*NK + ik (kappa fastest).  Units: mm, rad, 1/mm, T, GeV.
+ */
+#ifndef HOUGH_H_
+#define HOUGH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hough_ctx hough_ctx;
+
+typedef struct {
+    uint32_t n_phi0;               /* phi0 bins over [0, 2pi), centres (ip + 1/2) * 2pi/NPHI; >= 4                    */
+    uint32_t n_kappa;              /* kappa bins over [-kappa_max, +kappa_max), half-open; multiple of 8, >= 8        */
+    uint32_t n_d0;                 /* 1 -> prompt 2D mode (d0 == 0, kappa = 2 s / r); >= 2 -> 3D mode                 */
+    float    kappa_max;            /* 1/mm, > 0 (configs: 0.3e-3 * 3.8 / 1.0)                                         */
+    float    d0_min, d0_max;       /* mm; d0 bins over [d0_min, d0_max), centres; ignored in 2D mode                  */
+    float    b_tesla;              /* only used for pT = 0.3e-3 * B / |kappa|                                         */
+    uint32_t n_layers;             /* 1..16 (layer mask is 16 bits); hits with layer >= n_layers are ignored          */
+    uint32_t max_events;           /* per call, <= 1<<20                                                              */
+    uint64_t max_hits;             /* per call, total over events (sizes the prepared-hit workspace), < 2^32          */
+    uint32_t max_peaks_per_event;  /* capacity of the per-event peak / track lists                                    */
+    uint32_t max_jets_per_event;   /* capacity of the per-event jet list                                              */
+    uint32_t host_chunk_events;    /* hough_trigger_host only: events per internal chunk (the context then owns
+                                      2 * host_chunk_events * ND*NPHI*NK*2 bytes of accumulator planes); 0 disables   */
+} hough_config;
+
+typedef struct { uint32_t lin; uint16_t count; uint16_t mask; } hough_peak;                     /*  8 B */
+typedef struct { float pt, phi0, d0; int32_t q; int32_t jet; } hough_track;                     /* 20 B */
+typedef struct { uint32_t seed_track, n_tracks, n_displaced; float phi, sum_pt; } hough_jet;    /* 20 B */
+
+enum {
+    HOUGH_OK = 0,
+    HOUGH_EINVAL = -1,       /* bad config / null pointer / size over the configured maximum / bad scalar argument */
+    HOUGH_ECUDA = -2,        /* CUDA runtime error (text via hough_strerror)                                        */
+    HOUGH_ENOMEM = -3,       /* device allocation failed in hough_create                                            */
+    HOUGH_EUNSUPPORTED = -4  /* configuration valid but outside what the kernels are built for                      */
+};
+
+/* sticky status bits (hough_status) for conditions only visible on the device; they never trap */
+enum {
+    HOUGH_ST_EVENT_TOO_LARGE = 1u,   /* an event has > 65535 hits: its counts may wrap (uint16), results undefined  */
+    HOUGH_ST_BAD_OFFSETS = 2u,       /* hit_offsets not non-decreasing or beyond n_hits_total                        */
+    HOUGH_ST_TRIG_ROUNDING = 4u      /* informational: some sin/cos(phi) lay within a few fp64 ulps of an fp32
+                                        rounding boundary, so its correctly-rounded fp32 value is not certain
+                                        (reading R6; probability ~1e-8 per hit)                            */
+};
+
+/*
+ * Create a context.  HOST pointers.  Validates cfg, builds the constant tables in double precision
+ * (cos/sin of the phi0 bin centres, d0 bin centres, 2*d0, d0^2, NK/(2*kappa_max)), rounds each once to
+ * fp32, uploads them, and allocates the workspaces (prepared hits: 20 B per hit; peak bitmap: 1 bit per
+ * bin per event; jet keys: 8 B per stored peak; optional host-path planes).  Synchronous.
+ */
+int hough_create(const hough_config* cfg, hough_ctx** out);
+int hough_destroy(hough_ctx* ctx);
+
+/* bytes of ONE accumulator plane (count or mask) for n_events events: n_events * ND*NPHI*NK * 2 */
+size_t hough_plane_bytes(const hough_ctx* ctx, uint32_t n_events);
+
+/*
+ * A0-A2  Hough vote ("for each piece of input data votes are added to the feature instances that
+ * would include that input data"; "prompt or non-prompt tracks").  For every hit h of event e and
+ * every (id, ip): s = sin(phi_h - phi0c(ip)) (formed as sin(phi)cos(phi0c) - cos(phi)sin(phi0c) from
+ * correctly-rounded fp32 factors), kappa = 2 (r s + d0c) / (r^2 + 2 d0c r s + d0c^2)  (2D: 2 s / r), in IEEE
+ * fp32 without FMA in the fixed order of DESIGN.md O-2; if floor((kappa + kappa_max) * NK/(2 kappa_max)) is in
+ * [0, NK): count[e][id][ip][ik] += 1 and mask[e][id][ip][ik] |= 1 << layer_h.
+ *
+ *   d_hit_offsets [n_events+1] u32  CSR, non-decreasing.  off[0] is the base: hits of event e are the elements
+ *                 [off[e]-off[0], off[e+1]-off[0]) of d_r / d_phi / d_layer, so a sub-batch of a larger CSR batch
+ *                 is passed as (offsets + e0, r + off[e0], ...); off[n_events]-off[0] <= n_hits_total
+ *   d_r, d_phi    [n_hits_total] f32, d_layer [n_hits_total] u8   (r > 0 expected; any float is handled IEEE-wise)
+ *   d_count, d_mask [n_events][ND][NPHI][NK] u16 each, 16-byte aligned; FULLY overwritten (no memset needed)
+ * Precondition: <= 65535 hits per event (else HOUGH_ST_EVENT_TOO_LARGE is raised).
+ * Returns HOUGH_EINVAL if n_events > max_events or n_hits_total > max_hits or a pointer is null.
+ */
+int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets, uint64_t n_hits_total,
+               const float* d_r, const float* d_phi, const uint8_t* d_layer,
+               uint16_t* d_count, uint16_t* d_mask, void* stream);
+
+/*
+ * A3-A4  Peak finding + ordered compaction ("looking for local maxima in the parameter space").
+ * Bin b is a peak iff popcount(mask[b]) >= l_min and (count[b], -lin(b)) is strictly greatest over its 3x3
+ * (2D) / 3x3x3 (3D) neighbourhood; phi0 is periodic, kappa and d0 are clipped.  Peaks of each event are
+ * written in ascending lin.
+ *   d_peaks   [n_events][max_peaks_per_event]; only the first min(n_peaks[e], max_peaks) records are written
+ *   d_n_peaks [n_events] u32: the TRUE number of peaks found (may exceed the capacity)
+ * l_min must be in [1, n_layers].
+ */
+int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,
+                uint32_t l_min, hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream);
+
+/*
+ * A5-A6  Peak -> track conversion and phi-cone track-jets ("measure ... the transverse momentum";
+ * PAPER.md:113-123 jets / displaced jets, in north_star's phi-cone form).  For the T = min(n_peaks, max_peaks)
+ * stored peaks of each event: track j = {pT = 0.3e-3*B/|kappa_c|, phi0_c, d0_c, q = -sign(kappa_c), jet};
+ * seeded fixed-cone clustering on integer bin keys: seed = unassigned track with the smallest
+ * (|2 ik - (NK-1)|, j); members = unassigned tracks within floor(cone_rad*NPHI/2pi) phi0 bins (wrapped,
+ * inclusive); a track is displaced iff |d0_c| > d0_cut_mm; flag[e] = 1 iff some jet has
+ * n_displaced >= n_displaced_min.
+ *   d_tracks [n_events][max_peaks_per_event], d_jets [n_events][max_jets_per_event],
+ *   d_n_jets [n_events] u32 TRUE number of jets, d_flag [n_events] u8.
+ * Tracks of jets beyond the capacity keep jet = -1.
+ */
+int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+               float cone_rad, float d0_cut_mm, uint32_t n_displaced_min,
+               hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag, void* stream);
+
+/*
+ * End-to-end trigger on HOST buffers (the call bench.py's e2e leg times): copies the hits to the device,
+ * runs vote -> peaks -> jets in chunks of cfg.host_chunk_events events on the context's own planes, and
+ * copies n_peaks / n_jets / flag (and, if non-null, peaks and jets) back.  All h_* pointers are HOST memory
+ * (pinned memory makes the copies asynchronous); synchronises `stream` before returning.
+ * ms_stage (HOST, may be null) receives the device time in ms spent in {vote, peaks, jets}.
+ */
+int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
+                       const float* h_r, const float* h_phi, const uint8_t* h_layer,
+                       uint32_t l_min, float cone_rad, float d0_cut_mm, uint32_t n_displaced_min,
+                       uint32_t* h_n_peaks, uint32_t* h_n_jets, uint8_t* h_flag,
+                       hough_peak* h_peaks /* [n_events][max_peaks] or null */,
+                       hough_jet* h_jets /* [n_events][max_jets] or null */,
+                       float* ms_stage /* [3] or null */, void* stream);
+
+/* Synchronises the stream of the last call on ctx and returns (and keeps) the sticky status bits.  HOST out. */
+int hough_status(hough_ctx* ctx, uint32_t* host_status_bits);
+
+/* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches).  HOST out. */
+int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);
+
+/*
+ * Roofline micro-benchmarks: measured on the current device, synchronous.
+ *   kind 0: conflict-free 32-bit shared-memory atomics (add + or, result unused)   -> atomics / s
+ *   kind 1: dependent-free fp32 non-FMA arithmetic (FADD/FMUL)                      -> thread-instructions / s
+ *   kind 2: HBM read  (sum-reduce a buffer of `bytes`)                              -> bytes / s
+ *   kind 3: HBM write (fill a buffer of `bytes`)                                    -> bytes / s
+ * `bytes` is only used by kinds 2 and 3.  HOST out.
+ */
+int hough_microbench(int kind, size_t bytes, double* host_rate);
+
+const char* hough_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOUGH_H_ */

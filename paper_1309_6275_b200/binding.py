@@ -1,0 +1,220 @@
+"""Thin ctypes binding of libhough_b200.so -- argument marshalling only (include/hough.h is the contract).
+
+PyTorch is used for device memory and streams, nothing else: every step of the path (hit preparation, vote,
+peak stencil, compaction, tracks, jets) runs in the library's CUDA kernels.  There is no CPU fallback: if the
+shared library is missing or no CUDA device is present, loading / hough_create fail loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhough_b200.so")
+
+PEAK_DTYPE = np.dtype([("lin", "<u4"), ("count", "<u2"), ("mask", "<u2")])
+TRACK_DTYPE = np.dtype([("pt", "<f4"), ("phi0", "<f4"), ("d0", "<f4"), ("q", "<i4"), ("jet", "<i4")])
+JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced", "<u4"),
+                      ("phi", "<f4"), ("sum_pt", "<f4")])
+
+ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING = 1, 2, 4
+EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_jets",
+           "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror"]
+
+
+class HoughConfig(C.Structure):
+    _fields_ = [("n_phi0", C.c_uint32), ("n_kappa", C.c_uint32), ("n_d0", C.c_uint32),
+                ("kappa_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float), ("b_tesla", C.c_float),
+                ("n_layers", C.c_uint32), ("max_events", C.c_uint32), ("max_hits", C.c_uint64),
+                ("max_peaks_per_event", C.c_uint32), ("max_jets_per_event", C.c_uint32),
+                ("host_chunk_events", C.c_uint32)]
+
+
+class HoughError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} (code {code})")
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen the in-tree CUDA library; never falls back to anything else."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1309_6275_b200.build` "
+                "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        p, u32, u64, f32 = C.c_void_p, C.c_uint32, C.c_uint64, C.c_float
+        lib.hough_create.argtypes = [C.POINTER(HoughConfig), C.POINTER(p)]
+        lib.hough_destroy.argtypes = [p]
+        lib.hough_plane_bytes.argtypes = [p, u32]
+        lib.hough_plane_bytes.restype = C.c_size_t
+        lib.hough_vote.argtypes = [p, u32, p, u64, p, p, p, p, p, p]
+        lib.hough_peaks.argtypes = [p, u32, p, p, u32, p, p, p]
+        lib.hough_jets.argtypes = [p, u32, p, p, f32, f32, u32, p, p, p, p, p]
+        lib.hough_trigger_host.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, p, p, p, p, p, p, p]
+        lib.hough_status.argtypes = [p, C.POINTER(u32)]
+        lib.hough_launch_count.argtypes = [p, C.POINTER(u64)]
+        lib.hough_microbench.argtypes = [C.c_int, C.c_size_t, C.POINTER(C.c_double)]
+        lib.hough_strerror.argtypes = [C.c_int]
+        lib.hough_strerror.restype = C.c_char_p
+        for name in EXPORTS:
+            if name not in ("hough_plane_bytes", "hough_strerror"):
+                getattr(lib, name).restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return load_library().hough_strerror(code).decode()
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise HoughError(code, where)
+
+
+def microbench(kind: int, nbytes: int = 0) -> float:
+    """hough_microbench: 0 shared atomics/s, 1 fp32 non-FMA instr/s, 2 HBM read B/s, 3 HBM write B/s."""
+    out = C.c_double(0.0)
+    _check(load_library().hough_microbench(kind, nbytes, C.byref(out)), "hough_microbench")
+    return out.value
+
+
+def _dptr(t) -> C.c_void_p:
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream=None) -> C.c_void_p:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+class Hough:
+    """Owner of one hough_ctx.  Methods mirror the C entry points one to one (same names, same order)."""
+
+    def __init__(self, n_phi0: int, n_kappa: int, n_d0: int = 1, kappa_max: float = 0.3e-3 * 3.8,
+                 d0_min: float = 0.0, d0_max: float = 0.0, b_tesla: float = 3.8, n_layers: int = 8,
+                 max_events: int = 1, max_hits: int = 1 << 16, max_peaks_per_event: int = 4096,
+                 max_jets_per_event: int = 256, host_chunk_events: int = 0):
+        self.lib = load_library()
+        self.cfg = HoughConfig(n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, n_layers, max_events,
+                               max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events)
+        self._ctx = C.c_void_p()
+        _check(self.lib.hough_create(C.byref(self.cfg), C.byref(self._ctx)), "hough_create")
+
+    @classmethod
+    def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
+                     host_chunk_events: int = 0, max_peaks: Optional[int] = None) -> "Hough":
+        ne = w.n_events if max_events is None else max_events
+        mh = max_hits if max_hits is not None else ne * 65535
+        return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
+                   min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
+                   host_chunk_events)
+
+    # -- lifetime ---------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx:
+            self.lib.hough_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- sizes ------------------------------------------------------------------------------------
+    @property
+    def bins_per_event(self) -> int:
+        return self.cfg.n_d0 * self.cfg.n_phi0 * self.cfg.n_kappa
+
+    def hough_plane_bytes(self, n_events: int) -> int:
+        return int(self.lib.hough_plane_bytes(self._ctx, n_events))
+
+    def alloc_planes(self, n_events: int):
+        """Two uint16 device tensors [E, ND, NPHI, NK] (torch has no uint16 arithmetic; int16 storage is used)."""
+        import torch
+        shape = (n_events, self.cfg.n_d0, self.cfg.n_phi0, self.cfg.n_kappa)
+        return (torch.empty(shape, dtype=torch.int16, device="cuda"),
+                torch.empty(shape, dtype=torch.int16, device="cuda"))
+
+    def alloc_outputs(self, n_events: int):
+        import torch
+        mp, mj = self.cfg.max_peaks_per_event, self.cfg.max_jets_per_event
+        dev = "cuda"
+        return dict(
+            peaks=torch.zeros((n_events, mp, PEAK_DTYPE.itemsize), dtype=torch.uint8, device=dev),
+            n_peaks=torch.zeros(n_events, dtype=torch.int32, device=dev),
+            tracks=torch.zeros((n_events, mp, TRACK_DTYPE.itemsize), dtype=torch.uint8, device=dev),
+            jets=torch.zeros((n_events, mj, JET_DTYPE.itemsize), dtype=torch.uint8, device=dev),
+            n_jets=torch.zeros(n_events, dtype=torch.int32, device=dev),
+            flag=torch.zeros(n_events, dtype=torch.uint8, device=dev))
+
+    # -- the hot path (device pointers + caller stream) -------------------------------------------
+    def hough_vote(self, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, d_count, d_mask, stream=None):
+        _check(self.lib.hough_vote(self._ctx, n_events, _dptr(d_hit_offsets), n_hits_total, _dptr(d_r), _dptr(d_phi),
+                                   _dptr(d_layer), _dptr(d_count), _dptr(d_mask), _stream_ptr(stream)), "hough_vote")
+
+    def hough_peaks(self, n_events, d_count, d_mask, l_min, d_peaks, d_n_peaks, stream=None):
+        _check(self.lib.hough_peaks(self._ctx, n_events, _dptr(d_count), _dptr(d_mask), l_min, _dptr(d_peaks),
+                                    _dptr(d_n_peaks), _stream_ptr(stream)), "hough_peaks")
+
+    def hough_jets(self, n_events, d_peaks, d_n_peaks, cone_rad, d0_cut_mm, n_displaced_min, d_tracks, d_jets,
+                   d_n_jets, d_flag, stream=None):
+        _check(self.lib.hough_jets(self._ctx, n_events, _dptr(d_peaks), _dptr(d_n_peaks), cone_rad, d0_cut_mm,
+                                   n_displaced_min, _dptr(d_tracks), _dptr(d_jets), _dptr(d_n_jets), _dptr(d_flag),
+                                   _stream_ptr(stream)), "hough_jets")
+
+    def hough_trigger_host(self, n_events, h_hit_offsets, n_hits_total, h_r, h_phi, h_layer, l_min, cone_rad,
+                           d0_cut_mm, n_displaced_min, h_n_peaks, h_n_jets, h_flag, h_peaks=None, h_jets=None,
+                           ms_stage=None, stream=None):
+        """HOST tensors / arrays in and out (torch CPU tensors, ideally pinned, or numpy arrays)."""
+        def hp(x):
+            if x is None:
+                return C.c_void_p(0)
+            return C.c_void_p(x.ctypes.data) if isinstance(x, np.ndarray) else C.c_void_p(x.data_ptr())
+        _check(self.lib.hough_trigger_host(self._ctx, n_events, hp(h_hit_offsets), n_hits_total, hp(h_r), hp(h_phi),
+                                           hp(h_layer), l_min, cone_rad, d0_cut_mm, n_displaced_min, hp(h_n_peaks),
+                                           hp(h_n_jets), hp(h_flag), hp(h_peaks), hp(h_jets), hp(ms_stage),
+                                           _stream_ptr(stream)), "hough_trigger_host")
+
+    def hough_status(self) -> int:
+        out = C.c_uint32(0)
+        _check(self.lib.hough_status(self._ctx, C.byref(out)), "hough_status")
+        return out.value
+
+    def hough_launch_count(self) -> int:
+        out = C.c_uint64(0)
+        _check(self.lib.hough_launch_count(self._ctx, C.byref(out)), "hough_launch_count")
+        return out.value
+
+
+# -- conveniences used by tests / bench: upload a CSR batch, view raw output tensors as numpy records --------
+
+def upload_batch(batch):
+    """numpy CSR batch -> device tensors (offsets int32 storage of the uint32 values, r, phi, layer)."""
+    import torch
+    off = torch.from_numpy(batch.hit_offsets.view(np.int32)).cuda()
+    r = torch.from_numpy(batch.r).cuda()
+    phi = torch.from_numpy(batch.phi).cuda()
+    layer = torch.from_numpy(batch.layer).cuda()
+    return off, r, phi, layer
+
+
+def records(t, dtype: np.dtype) -> np.ndarray:
+    """Device uint8 tensor [..., itemsize] -> numpy structured array [...]."""
+    a = t.cpu().numpy()
+    return a.view(dtype).reshape(a.shape[:-1])
+
+
+def planes_to_numpy(t) -> np.ndarray:
+    return t.cpu().numpy().view(np.uint16)

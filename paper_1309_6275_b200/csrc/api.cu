@@ -1,0 +1,309 @@
+// C-ABI entry points of libhough_b200.so (see include/hough.h): validation, table construction, stream-ordered
+// launches.  No compute happens on the host; there is no CPU fallback.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "hough_internal.cuh"
+
+namespace {
+
+thread_local char g_errbuf[256] = "";
+
+int cuda_fail(cudaError_t err, const char* what)
+{
+    snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error in %s: %s", what, cudaGetErrorString(err));
+    return HOUGH_ECUDA;
+}
+
+#define CK(call, what)                                            \
+    do {                                                          \
+        cudaError_t err__ = (call);                               \
+        if (err__ != cudaSuccess) return cuda_fail(err__, what);  \
+    } while (0)
+
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t n)
+{
+    *p = nullptr;
+    if (n == 0) n = 1;
+    return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+}
+
+void free_all(hough_ctx* c)
+{
+    cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
+    cudaFree(c->d_rec); cudaFree(c->d_meta); cudaFree(c->d_layer_r); cudaFree(c->d_win); cudaFree(c->d_status);
+    cudaFree(c->d_bitmap); cudaFree(c->d_jetkeys);
+    cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
+    cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
+    cudaFree(c->d_hp_jets); cudaFree(c->d_hp_npeaks); cudaFree(c->d_hp_njets); cudaFree(c->d_hp_flag);
+    for (int i = 0; i < 4; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+}
+
+bool config_ok(const hough_config* g)
+{
+    if (g->n_phi0 < 4 || g->n_phi0 > (1u << 20)) return false;
+    if (g->n_kappa < 8 || g->n_kappa % 8 != 0 || g->n_kappa > (1u << 20)) return false;
+    if (g->n_d0 < 1 || g->n_d0 > (1u << 16)) return false;
+    if ((uint64_t)g->n_phi0 * g->n_kappa * g->n_d0 > 0xffffffffull) return false;      // lin is u32
+    if (!(g->kappa_max > 0.f) || !isfinite(g->kappa_max)) return false;
+    if (g->n_d0 > 1 && !(g->d0_max > g->d0_min && isfinite(g->d0_min) && isfinite(g->d0_max))) return false;
+    if (!isfinite(g->b_tesla)) return false;
+    if (g->n_layers < 1 || g->n_layers > HOUGH_MAX_LAYERS) return false;
+    if (g->max_events < 1 || g->max_events > (1u << 20)) return false;
+    if (g->max_hits < 1 || g->max_hits > 0xffffffffull) return false;
+    if (g->max_peaks_per_event < 1 || g->max_jets_per_event < 1) return false;
+    if (g->host_chunk_events > g->max_events) return false;
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* hough_strerror(int code)
+{
+    switch (code) {
+        case HOUGH_OK: return "ok";
+        case HOUGH_EINVAL: return "invalid argument";
+        case HOUGH_ECUDA: return g_errbuf[0] ? g_errbuf : "CUDA runtime error";
+        case HOUGH_ENOMEM: return "device allocation failed";
+        case HOUGH_EUNSUPPORTED: return "configuration not supported by the kernels";
+    }
+    return "unknown error code";
+}
+
+int hough_create(const hough_config* cfg, hough_ctx** out)
+{
+    if (!cfg || !out) return HOUGH_EINVAL;
+    *out = nullptr;
+    if (!config_ok(cfg)) return HOUGH_EINVAL;
+    int dev = 0;
+    CK(cudaGetDevice(&dev), "cudaGetDevice");
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties");
+    if (prop.major < 10) {
+        snprintf(g_errbuf, sizeof(g_errbuf), "device sm_%d%d is not sm_100-class", prop.major, prop.minor);
+        return HOUGH_ECUDA;
+    }
+    hough_ctx* c = new (std::nothrow) hough_ctx();
+    if (!c) return HOUGH_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->cfg = *cfg;
+    c->device = dev;
+    c->sm_count = prop.multiProcessorCount;
+    if (plan_vote(c) != cudaSuccess || plan_peaks(c) != cudaSuccess) { delete c; return HOUGH_EUNSUPPORTED; }
+
+    // O-0 tables: double precision, each value rounded once to fp32
+    const uint32_t NP = cfg->n_phi0, ND = cfg->n_d0, NK = cfg->n_kappa;
+    std::vector<float> c0(NP), s0(NP), d0c(ND), two_d0(ND), d0sq(ND);
+    const double pi = 3.14159265358979323846;
+    for (uint32_t ip = 0; ip < NP; ++ip) {
+        const double ph = ((double)ip + 0.5) * (2.0 * pi / (double)NP);
+        c0[ip] = (float)cos(ph);
+        s0[ip] = (float)sin(ph);
+    }
+    for (uint32_t id = 0; id < ND; ++id) {
+        float d = 0.f;
+        if (ND > 1)
+            d = (float)((double)cfg->d0_min + ((double)id + 0.5) * (((double)cfg->d0_max - (double)cfg->d0_min) / (double)ND));
+        volatile float dd = d * d;                    // one fp32 multiply, kept out of any contraction
+        d0c[id] = d; two_d0[id] = 2.0f * d; d0sq[id] = dd;
+    }
+    c->kmax = cfg->kappa_max;
+    c->inv_dk = (float)((double)NK / (2.0 * (double)cfg->kappa_max));
+    c->nk_f = (float)NK;
+
+    const size_t bins = (size_t)ND * NP * NK;
+    cudaError_t err = cudaSuccess;
+    auto A = [&](cudaError_t e2) { if (err == cudaSuccess) err = e2; };
+    A(dev_alloc(&c->d_c0, NP)); A(dev_alloc(&c->d_s0, NP));
+    A(dev_alloc(&c->d_d0c, ND)); A(dev_alloc(&c->d_two_d0, ND)); A(dev_alloc(&c->d_d0sq, ND));
+    A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_meta, cfg->max_hits));
+    A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS)); A(dev_alloc(&c->d_win, (size_t)HOUGH_MAX_LAYERS * ND));
+    A(dev_alloc(&c->d_status, 2));
+    A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
+    A(dev_alloc(&c->d_jetkeys, (size_t)cfg->max_events * cfg->max_peaks_per_event));
+    if (cfg->host_chunk_events > 0) {
+        const size_t E = cfg->max_events, H = cfg->max_hits;
+        A(dev_alloc(&c->d_hp_count, (size_t)cfg->host_chunk_events * bins));
+        A(dev_alloc(&c->d_hp_mask, (size_t)cfg->host_chunk_events * bins));
+        A(dev_alloc(&c->d_hp_off, E + 1)); A(dev_alloc(&c->d_hp_r, H)); A(dev_alloc(&c->d_hp_phi, H));
+        A(dev_alloc(&c->d_hp_layer, H));
+        A(dev_alloc(&c->d_hp_peaks, E * cfg->max_peaks_per_event));
+        A(dev_alloc(&c->d_hp_tracks, E * cfg->max_peaks_per_event));
+        A(dev_alloc(&c->d_hp_jets, E * cfg->max_jets_per_event));
+        A(dev_alloc(&c->d_hp_npeaks, E)); A(dev_alloc(&c->d_hp_njets, E)); A(dev_alloc(&c->d_hp_flag, E));
+    }
+    if (err != cudaSuccess) {
+        cuda_fail(err, "hough_create allocation");
+        free_all(c); delete c;
+        cudaGetLastError();
+        return (err == cudaErrorMemoryAllocation) ? HOUGH_ENOMEM : HOUGH_ECUDA;
+    }
+    uint32_t lr[2 * HOUGH_MAX_LAYERS];
+    for (int i = 0; i < HOUGH_MAX_LAYERS; ++i) { lr[i] = 0x7f800000u; lr[HOUGH_MAX_LAYERS + i] = 0u; }
+    A(cudaMemcpy(c->d_c0, c0.data(), NP * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_s0, s0.data(), NP * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_d0c, d0c.data(), ND * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_two_d0, two_d0.data(), ND * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_d0sq, d0sq.data(), ND * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
+    A(cudaMemset(c->d_status, 0, 8));
+    for (int i = 0; i < 4; ++i) A(cudaEventCreate(&c->ev[i]));
+    if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
+    *out = c;
+    return HOUGH_OK;
+}
+
+int hough_destroy(hough_ctx* ctx)
+{
+    if (!ctx) return HOUGH_EINVAL;
+    cudaDeviceSynchronize();
+    free_all(ctx);
+    delete ctx;
+    return HOUGH_OK;
+}
+
+size_t hough_plane_bytes(const hough_ctx* ctx, uint32_t n_events)
+{
+    if (!ctx) return 0;
+    return (size_t)n_events * ctx->cfg.n_d0 * ctx->cfg.n_phi0 * ctx->cfg.n_kappa * 2;
+}
+
+int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets, uint64_t n_hits_total,
+               const float* d_r, const float* d_phi, const uint8_t* d_layer, uint16_t* d_count, uint16_t* d_mask,
+               void* stream)
+{
+    if (!ctx || !d_hit_offsets || !d_count || !d_mask) return HOUGH_EINVAL;
+    if (n_hits_total > 0 && (!d_r || !d_phi || !d_layer)) return HOUGH_EINVAL;
+    if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
+    if (((uintptr_t)d_count | (uintptr_t)d_mask) & 15u) return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    if (n_events == 0) return HOUGH_OK;
+    CK(launch_prep(ctx, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, st), "hit preparation");
+    CK(launch_vote(ctx, n_events, d_hit_offsets, d_hit_offsets, d_count, d_mask, st), "vote kernel");
+    return HOUGH_OK;
+}
+
+int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask, uint32_t l_min,
+                hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream)
+{
+    if (!ctx || !d_count || !d_mask || !d_peaks || !d_n_peaks) return HOUGH_EINVAL;
+    if (n_events > ctx->cfg.max_events || l_min < 1 || l_min > ctx->cfg.n_layers) return HOUGH_EINVAL;
+    if (((uintptr_t)d_count | (uintptr_t)d_mask) & 15u) return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    CK(launch_peaks(ctx, n_events, d_count, d_mask, l_min, d_peaks, d_n_peaks, st), "peak kernels");
+    return HOUGH_OK;
+}
+
+static int cone_bins_of(float cone_rad, uint32_t n_phi0)
+{
+    const double pi = 3.14159265358979323846;
+    double b = floor((double)cone_rad * (double)n_phi0 / (2.0 * pi));
+    if (b > (double)n_phi0) b = (double)n_phi0;
+    return (int)b;
+}
+
+int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks, float cone_rad,
+               float d0_cut_mm, uint32_t n_displaced_min, hough_track* d_tracks, hough_jet* d_jets,
+               uint32_t* d_n_jets, uint8_t* d_flag, void* stream)
+{
+    if (!ctx || !d_peaks || !d_n_peaks || !d_tracks || !d_jets || !d_n_jets || !d_flag) return HOUGH_EINVAL;
+    if (n_events > ctx->cfg.max_events || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm)) return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    CK(launch_jets(ctx, n_events, d_peaks, d_n_peaks, cone_bins_of(cone_rad, ctx->cfg.n_phi0), d0_cut_mm,
+                   n_displaced_min, d_tracks, d_jets, d_n_jets, d_flag, st), "jet kernel");
+    return HOUGH_OK;
+}
+
+int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
+                       const float* h_r, const float* h_phi, const uint8_t* h_layer, uint32_t l_min, float cone_rad,
+                       float d0_cut_mm, uint32_t n_displaced_min, uint32_t* h_n_peaks, uint32_t* h_n_jets,
+                       uint8_t* h_flag, hough_peak* h_peaks, hough_jet* h_jets, float* ms_stage, void* stream)
+{
+    if (!ctx || !h_hit_offsets || !h_n_peaks || !h_n_jets || !h_flag) return HOUGH_EINVAL;
+    if (ctx->cfg.host_chunk_events == 0) return HOUGH_EINVAL;
+    if (n_hits_total > 0 && (!h_r || !h_phi || !h_layer)) return HOUGH_EINVAL;
+    if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
+    if (l_min < 1 || l_min > ctx->cfg.n_layers || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm))
+        return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    if (ms_stage) ms_stage[0] = ms_stage[1] = ms_stage[2] = 0.f;
+    if (n_events == 0) return HOUGH_OK;
+    const hough_config& g = ctx->cfg;
+    CK(cudaMemcpyAsync(ctx->d_hp_off, h_hit_offsets, ((size_t)n_events + 1) * 4, cudaMemcpyHostToDevice, st), "H2D offsets");
+    if (n_hits_total) {
+        CK(cudaMemcpyAsync(ctx->d_hp_r, h_r, n_hits_total * 4, cudaMemcpyHostToDevice, st), "H2D r");
+        CK(cudaMemcpyAsync(ctx->d_hp_phi, h_phi, n_hits_total * 4, cudaMemcpyHostToDevice, st), "H2D phi");
+        CK(cudaMemcpyAsync(ctx->d_hp_layer, h_layer, n_hits_total, cudaMemcpyHostToDevice, st), "H2D layer");
+    }
+    // hits are prepared once for the whole batch; the chunks then share the prepared records
+    CK(launch_prep(ctx, n_events, ctx->d_hp_off, n_hits_total, ctx->d_hp_r, ctx->d_hp_phi, ctx->d_hp_layer, st), "hit preparation");
+    const int cone_bins = cone_bins_of(cone_rad, g.n_phi0);
+    std::vector<cudaEvent_t> evs;
+    for (uint32_t e0 = 0; e0 < n_events; e0 += g.host_chunk_events) {
+        const uint32_t ne = (n_events - e0 < g.host_chunk_events) ? n_events - e0 : g.host_chunk_events;
+        cudaEvent_t t[4] = {nullptr, nullptr, nullptr, nullptr};
+        if (ms_stage) for (int i = 0; i < 4; ++i) { CK(cudaEventCreate(&t[i]), "event"); evs.push_back(t[i]); }
+        if (ms_stage) cudaEventRecord(t[0], st);
+        CK(launch_vote(ctx, ne, ctx->d_hp_off + e0, ctx->d_hp_off, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel");
+        if (ms_stage) cudaEventRecord(t[1], st);
+        CK(launch_peaks(ctx, ne, ctx->d_hp_count, ctx->d_hp_mask, l_min, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event,
+                        ctx->d_hp_npeaks + e0, st), "peak kernels");
+        if (ms_stage) cudaEventRecord(t[2], st);
+        CK(launch_jets(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, cone_bins,
+                       d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e0 * g.max_peaks_per_event,
+                       ctx->d_hp_jets + (size_t)e0 * g.max_jets_per_event, ctx->d_hp_njets + e0, ctx->d_hp_flag + e0, st),
+           "jet kernel");
+        if (ms_stage) cudaEventRecord(t[3], st);
+    }
+    CK(cudaMemcpyAsync(h_n_peaks, ctx->d_hp_npeaks, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks");
+    CK(cudaMemcpyAsync(h_n_jets, ctx->d_hp_njets, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_jets");
+    CK(cudaMemcpyAsync(h_flag, ctx->d_hp_flag, (size_t)n_events, cudaMemcpyDeviceToHost, st), "D2H flag");
+    if (h_peaks)
+        CK(cudaMemcpyAsync(h_peaks, ctx->d_hp_peaks, (size_t)n_events * g.max_peaks_per_event * sizeof(hough_peak),
+                           cudaMemcpyDeviceToHost, st), "D2H peaks");
+    if (h_jets)
+        CK(cudaMemcpyAsync(h_jets, ctx->d_hp_jets, (size_t)n_events * g.max_jets_per_event * sizeof(hough_jet),
+                           cudaMemcpyDeviceToHost, st), "D2H jets");
+    CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
+    if (ms_stage) {
+        for (size_t i = 0; i + 3 < evs.size(); i += 4)
+            for (int s = 0; s < 3; ++s) {
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, evs[i + s], evs[i + s + 1]);
+                ms_stage[s] += ms;
+            }
+    }
+    for (cudaEvent_t ev : evs) cudaEventDestroy(ev);
+    return HOUGH_OK;
+}
+
+int hough_status(hough_ctx* ctx, uint32_t* host_status_bits)
+{
+    if (!ctx || !host_status_bits) return HOUGH_EINVAL;
+    CK(cudaStreamSynchronize(ctx->last_stream), "hough_status synchronize");
+    uint32_t st[2] = {0, 0};
+    CK(cudaMemcpy(st, ctx->d_status, 8, cudaMemcpyDeviceToHost), "hough_status copy");
+    ctx->status_host |= st[0];
+    *host_status_bits = ctx->status_host;
+    return HOUGH_OK;
+}
+
+int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count)
+{
+    if (!ctx || !host_count) return HOUGH_EINVAL;
+    *host_count = ctx->launches;
+    return HOUGH_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// Internal declarations shared by the translation units of libhough_b200.so (sm_100a only).
+// Nothing here is visible across the C-ABI (include/hough.h) and nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "hough.h"
+
+#define HOUGH_MAX_LAYERS 16
+#define HOUGH_TILE_W 32              // phi0 columns per vote tile = lanes of a warp
+
+// meta word of a prepared hit: bits 0..19 phi bucket pb (0 <= pb < NPHI), bits 20..23 layer,
+// bit 30 "wild" (r not a positive finite number: no window pruning), bit 31 "dropped" (never votes).
+#define META_PB_MASK 0xFFFFFu
+#define META_LAYER_SHIFT 20
+#define META_WILD (1u << 30)
+#define META_DROP (1u << 31)
+
+// pruning window of (layer, id): columns ip that can receive a vote from a hit in phi bucket pb satisfy
+// ip - pb in [lo1, hi1] or [lo2, hi2] (mod NPHI).  lo > hi encodes "empty".
+struct Window { int lo1, hi1, lo2, hi2; };
+
+struct VotePlan {
+    int ids_per_tile;                // K: d0 bins per tile (1..4)
+    int nk_tile;                     // kappa bins per tile (<= NK; NK split into nk_seg segments if it does not fit)
+    int nk_seg;
+    int threads;
+    int list_cap;                    // staged-hit list capacity (records)
+    size_t smem_bytes;
+    int n_strips, n_tiles;           // ceil(ND/K), ceil(NPHI/32)
+};
+
+struct PeakPlan {
+    int tp;                          // phi0 rows per stencil tile
+    int threads;
+    size_t smem_bytes;
+    int n_tiles;
+};
+
+struct hough_ctx {
+    hough_config cfg;
+    int device;
+    int sm_count;
+    // constant tables (device), fp32 rounded once from double
+    float* d_c0; float* d_s0;                 // [NPHI]
+    float* d_d0c; float* d_two_d0; float* d_d0sq;   // [ND]
+    float kmax, inv_dk, nk_f;
+    // per-call workspace
+    float4* d_rec;                            // [max_hits] {sin phi, cos phi, r, meta}
+    uint32_t* d_meta;                         // [max_hits]
+    uint32_t* d_layer_r;                      // [2*16] float bits: min r, max r per layer
+    Window* d_win;                            // [16][ND]
+    uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
+    uint8_t* d_bitmap;                        // [max_events][bins/8]
+    uint64_t* d_jetkeys;                      // [max_events][max_peaks]
+    // host path
+    uint16_t* d_hp_count; uint16_t* d_hp_mask;     // [host_chunk_events][bins]
+    uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
+    hough_peak* d_hp_peaks; hough_track* d_hp_tracks; hough_jet* d_hp_jets;
+    uint32_t* d_hp_npeaks; uint32_t* d_hp_njets; uint8_t* d_hp_flag;
+    cudaEvent_t ev[4];
+    VotePlan vote;
+    PeakPlan peak;
+    cudaStream_t last_stream;
+    uint64_t launches;
+    uint32_t status_host;
+};
+
+// launchers (each returns a cudaError_t from the launch; all asynchronous on `st`)
+cudaError_t launch_prep(hough_ctx* c, uint32_t n_events, const uint32_t* d_off, uint64_t n_hits,
+                        const float* d_r, const float* d_phi, const uint8_t* d_layer, cudaStream_t st);
+cudaError_t launch_vote(hough_ctx* c, uint32_t n_events, const uint32_t* d_off, const uint32_t* d_base,
+                        uint16_t* d_count, uint16_t* d_mask, cudaStream_t st);
+cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,
+                         uint32_t l_min, hough_peak* d_peaks, uint32_t* d_n_peaks, cudaStream_t st);
+cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                        int cone_bins, float d0_cut, uint32_t n_min, hough_track* d_tracks, hough_jet* d_jets,
+                        uint32_t* d_n_jets, uint8_t* d_flag, cudaStream_t st);
+cudaError_t plan_vote(hough_ctx* c);
+cudaError_t plan_peaks(hough_ctx* c);

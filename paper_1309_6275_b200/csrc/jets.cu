@@ -1,0 +1,136 @@
+// A5 peak -> track conversion and A6 seeded phi-cone track-jets, one warp per event (sm_100a).
+//
+// DESIGN.md O-4 / O-5 (PAPER.md:87 transverse-momentum measurement; PAPER.md:113-123 jets and the
+// interaction-point remark; clustering rule from north_star as read in R17-R22).  All decisions are taken on
+// integer bin keys; floats only appear in the reported fields (tolerance 1e-5).
+#include "hough_internal.cuh"
+
+namespace {
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr uint64_t KEY_ASSIGNED = 1ull << 63;
+
+struct JetParams {
+    const hough_peak* peaks; const uint32_t* n_peaks;
+    hough_track* tracks; hough_jet* jets; uint32_t* n_jets; uint8_t* flag;
+    uint64_t* keys;
+    const float* d0c;
+    uint32_t n_events, max_peaks, max_jets;
+    int n_d0, n_phi0, n_kappa;
+    float kmax, b_tesla, d0_cut;
+    int cone_bins;
+    uint32_t n_min;
+};
+
+__device__ __forceinline__ uint64_t warp_min_u64(uint64_t v)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        const uint64_t o = __shfl_xor_sync(0xffffffffu, v, d);
+        v = (o < v) ? o : v;
+    }
+    return v;
+}
+
+__global__ void __launch_bounds__(128) jets_kernel(const JetParams p)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (e >= p.n_events) return;
+    const uint32_t T = min(p.n_peaks[e], p.max_peaks);
+    const hough_peak* pk = p.peaks + (size_t)e * p.max_peaks;
+    hough_track* trk = p.tracks + (size_t)e * p.max_peaks;
+    hough_jet* jets = p.jets + (size_t)e * p.max_jets;
+    uint64_t* keys = p.keys + (size_t)e * p.max_peaks;
+    const int NK = p.n_kappa, N = p.n_phi0;
+    const double kmax = (double)p.kmax;
+
+    // A5: tracks, and the integer keys of the clustering: [63] assigned, [32..55] a = |2 ik - (NK-1)|,
+    // [1..21] ip, [0] displaced
+    for (uint32_t j = lane; j < T; j += 32) {
+        const uint32_t lin = pk[j].lin;
+        const uint32_t ik = lin % (uint32_t)NK, t = lin / (uint32_t)NK;
+        const uint32_t ip = t % (uint32_t)N, id = t / (uint32_t)N;
+        const double kc = -kmax + ((double)ik + 0.5) * (2.0 * kmax / (double)NK);
+        hough_track tr;
+        tr.pt = (float)(0.3e-3 * (double)p.b_tesla / fabs(kc));
+        tr.phi0 = (float)(((double)ip + 0.5) * (kTwoPi / (double)N));
+        const float d0 = (p.n_d0 > 1) ? p.d0c[id] : 0.0f;
+        tr.d0 = d0;
+        tr.q = (kc < 0.0) ? +1 : -1;
+        tr.jet = -1;
+        trk[j] = tr;
+        const uint32_t a = (uint32_t)abs(2 * (int)ik - (NK - 1));
+        const uint32_t disp = (p.n_d0 > 1 && fabsf(d0) > p.d0_cut) ? 1u : 0u;
+        keys[j] = ((uint64_t)a << 32) | ((uint64_t)ip << 1) | disp;
+    }
+    __syncwarp();
+
+    // A6: repeat { seed = unassigned track with the smallest (a, j); members = unassigned within the cone }
+    uint32_t J = 0;
+    bool any_flag = false;
+    for (;;) {
+        uint64_t best = ~0ull;
+        for (uint32_t j = lane; j < T; j += 32) {
+            const uint64_t k = keys[j];
+            if (!(k & KEY_ASSIGNED)) {
+                const uint64_t cand = (k & 0x00ffffff00000000ull) | j;
+                best = (cand < best) ? cand : best;
+            }
+        }
+        best = warp_min_u64(best);
+        if (best == ~0ull) break;
+        const uint32_t seed = (uint32_t)(best & 0xffffffffu);
+        const int ip_seed = (int)((keys[seed] >> 1) & 0xfffffu);
+        uint32_t n_tracks = 0, n_disp = 0;
+        double sum_pt = 0.0;
+        for (uint32_t j = lane; j < T; j += 32) {
+            const uint64_t k = keys[j];
+            if (k & KEY_ASSIGNED) continue;
+            int d = abs((int)((k >> 1) & 0xfffffu) - ip_seed);
+            d = min(d, N - d);
+            if (d <= p.cone_bins) {
+                keys[j] = k | KEY_ASSIGNED;
+                ++n_tracks;
+                n_disp += (uint32_t)(k & 1u);
+                sum_pt += (double)trk[j].pt;
+                if (J < p.max_jets) trk[j].jet = (int32_t)J;
+            }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            n_tracks += __shfl_xor_sync(0xffffffffu, n_tracks, d);
+            n_disp += __shfl_xor_sync(0xffffffffu, n_disp, d);
+            sum_pt += __shfl_xor_sync(0xffffffffu, sum_pt, d);
+        }
+        if (lane == 0 && J < p.max_jets) {
+            hough_jet jt;
+            jt.seed_track = seed; jt.n_tracks = n_tracks; jt.n_displaced = n_disp;
+            jt.phi = trk[seed].phi0; jt.sum_pt = (float)sum_pt;
+            jets[J] = jt;
+        }
+        any_flag = any_flag || (n_disp >= p.n_min);
+        ++J;
+    }
+    if (lane == 0) { p.n_jets[e] = J; p.flag[e] = any_flag ? 1 : 0; }
+}
+
+}  // namespace
+
+cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                        int cone_bins, float d0_cut, uint32_t n_min, hough_track* d_tracks, hough_jet* d_jets,
+                        uint32_t* d_n_jets, uint8_t* d_flag, cudaStream_t st)
+{
+    if (n_events == 0) return cudaSuccess;
+    JetParams p;
+    p.peaks = d_peaks; p.n_peaks = d_n_peaks; p.tracks = d_tracks; p.jets = d_jets; p.n_jets = d_n_jets;
+    p.flag = d_flag; p.keys = c->d_jetkeys; p.d0c = c->d_d0c;
+    p.n_events = n_events; p.max_peaks = c->cfg.max_peaks_per_event; p.max_jets = c->cfg.max_jets_per_event;
+    p.n_d0 = (int)c->cfg.n_d0; p.n_phi0 = (int)c->cfg.n_phi0; p.n_kappa = (int)c->cfg.n_kappa;
+    p.kmax = c->kmax; p.b_tesla = c->cfg.b_tesla; p.d0_cut = d0_cut; p.cone_bins = cone_bins; p.n_min = n_min;
+    const uint32_t warps_per_block = 4;
+    jets_kernel<<<(n_events + warps_per_block - 1) / warps_per_block, warps_per_block * 32, 0, st>>>(p);
+    ++c->launches;
+    return cudaGetLastError();
+}

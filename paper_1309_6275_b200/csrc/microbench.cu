@@ -1,0 +1,116 @@
+// Roofline micro-benchmarks: the denominators the vote kernel and the stencil are
+// reported against are measured on the box, not assumed.  Synchronous helpers; not part of the hot path.
+#include <stdio.h>
+
+#include "hough_internal.cuh"
+
+namespace {
+
+// kind 0: conflict-free 32-bit shared atomics, one add + one or per step, result unused (the vote's pattern)
+__global__ void __launch_bounds__(1024) mb_shared_atomics(int iters, uint32_t* sink)
+{
+    __shared__ uint32_t s[8192];
+    for (int i = threadIdx.x; i < 8192; i += blockDim.x) s[i] = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t idx = (warp * 97u) & 255u;                  // row of 32 words; lanes hit 32 distinct banks
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            uint32_t* w = &s[((idx + u * 13u) & 255u) * 32u + lane];
+            atomicAdd(w, 1u);
+            atomicOr(w, 0x10000u);
+        }
+        idx += 7u;
+    }
+    __syncthreads();
+    if (s[threadIdx.x] == 0xdeadbeefu) sink[0] = 1;
+}
+
+// kind 1: fp32 non-FMA arithmetic, 8 independent chains per thread
+__global__ void __launch_bounds__(1024) mb_fp32(int iters, float seed, float* sink)
+{
+    float a0 = seed + threadIdx.x, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f;
+    float a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f, a7 = a0 + 7.f;
+    const float m = 0.999999f, c = 1e-3f;
+    for (int i = 0; i < iters; ++i) {
+        a0 = __fmul_rn(a0, m); a1 = __fadd_rn(a1, c); a2 = __fmul_rn(a2, m); a3 = __fadd_rn(a3, c);
+        a4 = __fmul_rn(a4, m); a5 = __fadd_rn(a5, c); a6 = __fmul_rn(a6, m); a7 = __fadd_rn(a7, c);
+        a0 = __fadd_rn(a0, c); a1 = __fmul_rn(a1, m); a2 = __fadd_rn(a2, c); a3 = __fmul_rn(a3, m);
+        a4 = __fadd_rn(a4, c); a5 = __fmul_rn(a5, m); a6 = __fadd_rn(a6, c); a7 = __fmul_rn(a7, m);
+    }
+    const float r = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (r == 12345.678f) sink[0] = r;
+}
+
+__global__ void __launch_bounds__(512) mb_read(const uint4* __restrict__ src, size_t n16, uint32_t* sink)
+{
+    uint32_t acc = 0;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n16; i += 4 * stride) {
+        const uint4 a = src[i], b = src[i + stride], c = src[i + 2 * stride], d = src[i + 3 * stride];
+        acc += a.x ^ a.y ^ a.z ^ a.w ^ b.x ^ b.y ^ b.z ^ b.w ^ c.x ^ c.y ^ c.z ^ c.w ^ d.x ^ d.y ^ d.z ^ d.w;
+    }
+    for (; i < n16; i += stride) { const uint4 a = src[i]; acc += a.x ^ a.y ^ a.z ^ a.w; }
+    if (acc == 0x12345u) sink[0] = acc;
+}
+
+__global__ void __launch_bounds__(512) mb_write(uint4* __restrict__ dst, size_t n16)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride)
+        dst[i] = make_uint4((uint32_t)i, 1u, 2u, 3u);
+}
+
+}  // namespace
+
+extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
+{
+    if (!host_rate || kind < 0 || kind > 3) return HOUGH_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ECUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    uint32_t* sink = nullptr;
+    cudaMalloc((void**)&sink, 16);
+    void* buf = nullptr;
+    double work = 0.0;
+    float best_ms = 1e30f;
+    const int reps = 5;
+    if (kind >= 2) {
+        if (bytes < (1u << 20)) bytes = (size_t)1 << 30;
+        if (cudaMalloc(&buf, bytes) != cudaSuccess) { cudaFree(sink); return HOUGH_ENOMEM; }
+        cudaMemset(buf, 1, bytes);
+    }
+    for (int rep = 0; rep < reps + 1; ++rep) {
+        cudaEventRecord(t0);
+        if (kind == 0) {
+            const int iters = 4096;
+            mb_shared_atomics<<<sms * 2, 1024>>>(iters, sink);
+            work = (double)sms * 2 * 1024 * iters * 16;
+        } else if (kind == 1) {
+            const int iters = 8192;
+            mb_fp32<<<sms * 2, 1024>>>(iters, 1.0f, (float*)sink);
+            work = (double)sms * 2 * 1024 * iters * 16;
+        } else if (kind == 2) {
+            mb_read<<<sms * 8, 512>>>((const uint4*)buf, bytes / 16, sink);
+            work = (double)bytes;
+        } else {
+            mb_write<<<sms * 8, 512>>>((uint4*)buf, bytes / 16);
+            work = (double)bytes;
+        }
+        cudaEventRecord(t1);
+        cudaEventSynchronize(t1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaError_t err = cudaGetLastError();
+    cudaFree(buf); cudaFree(sink);
+    cudaEventDestroy(t0); cudaEventDestroy(t1);
+    if (err != cudaSuccess) return HOUGH_ECUDA;
+    *host_rate = work / ((double)best_ms * 1e-3);
+    return HOUGH_OK;
+}

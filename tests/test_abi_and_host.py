@@ -1,0 +1,154 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol include/hough.h
+declares, the ctypes struct matches the header layout, the generators are deterministic, and the event-sharding
+logic used for N > 1 GPUs is exercised with a world_size-2 gloo group (no compute calls without a GPU)."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "hough.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(hough_[a-z_]+)\s*\(", text)))
+
+
+def test_library_builds_loads_and_exports_every_declared_symbol():
+    from paper_1309_6275_b200 import build, binding
+    build.build()
+    lib = C.CDLL(binding.LIB_PATH)
+    declared = _declared_symbols()
+    assert set(declared) == set(binding.EXPORTS), (declared, binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    # only sm_100a code is embedded
+    out = subprocess.run(["cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "sm_100a" in out and not re.search(r"sm_(?!100a)\d+", out), out
+
+
+def test_strerror_and_argument_validation_without_gpu():
+    from paper_1309_6275_b200 import binding as B
+    lib = B.load_library()
+    assert B.strerror(0) == "ok" and "invalid" in B.strerror(-1)
+    # a bad config is rejected before any CUDA call; null pointers likewise
+    ctx = C.c_void_p()
+    bad = B.HoughConfig(512, 250, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0)          # n_kappa % 8 != 0
+    assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
+    bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0)        # n_layers > 16
+    assert lib.hough_create(C.byref(bad2), C.byref(ctx)) == -1
+    assert lib.hough_create(None, C.byref(ctx)) == -1
+    assert lib.hough_destroy(None) == -1
+    assert lib.hough_plane_bytes(None, 3) == 0
+
+
+def test_config_struct_layout_matches_header():
+    from paper_1309_6275_b200 import binding as B
+    # compile a 3-line C program against the real header and compare sizeof / offsets
+    src = r'''
+    #include <stdio.h>
+    #include <stddef.h>
+    #include "hough.h"
+    int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(hough_config), offsetof(hough_config, max_hits),
+        offsetof(hough_config, host_chunk_events), sizeof(hough_peak), sizeof(hough_track), sizeof(hough_jet),
+        offsetof(hough_config, max_events)); return 0; }'''
+    exe = os.path.join(ROOT, "_work", "layout_probe") if os.path.isdir(os.path.join(ROOT, "_work")) else "/tmp/layout_probe"
+    exe = "/tmp/hough_layout_probe"
+    subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=src, text=True, check=True)
+    vals = list(map(int, subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()))
+    assert vals[0] == C.sizeof(B.HoughConfig)
+    assert vals[1] == B.HoughConfig.max_hits.offset and vals[2] == B.HoughConfig.host_chunk_events.offset
+    assert vals[6] == B.HoughConfig.max_events.offset
+    assert vals[3] == B.PEAK_DTYPE.itemsize == 8 and vals[4] == B.TRACK_DTYPE.itemsize == 20
+    assert vals[5] == B.JET_DTYPE.itemsize == 20
+
+
+def test_product_path_never_touches_the_oracle():
+    """No file of the package (or bench's product arm) imports oracle/; the oracle never imports the package."""
+    pkg = os.path.join(ROOT, "paper_1309_6275_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "hough_oracle" not in text and "from oracle" not in text and "import oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_1309_6275_b200 import" not in text and "import paper_1309_6275_b200" not in text
+            assert "hough.h" not in text
+
+
+def test_generators_are_deterministic_and_shaped_like_the_configs():
+    from paper_1309_6275_b200 import workloads as W
+    a = W.generate(W.config(1)); b = W.generate(W.config(1))
+    assert a.n_hits == 180 and np.array_equal(a.phi, b.phi) and np.array_equal(a.layer, b.layer)
+    assert a.r.dtype == np.float32 and a.layer.dtype == np.uint8 and a.hit_offsets.dtype == np.uint32
+    assert set(np.unique(a.r).tolist()) <= set(np.float32(W.TRACKER_A).tolist())
+    assert np.all((a.phi >= 0) & (a.phi <= np.float32(2 * np.pi)))
+    c3 = W.generate(W.config(3), 3)
+    assert c3.n_events == 3 and np.all(np.diff(c3.hit_offsets.astype(np.int64)) == 2600)
+    c4 = W.generate(W.config(4), 2, keep_truth=True)
+    assert 9000 < c4.n_hits / 2 < 9500 and c4.layer.max() == 11
+    for t in c4.truth:
+        assert t["n_vertices"] == 3 and 18 <= t["disp_kappa"].size <= 36
+    c5 = W.generate(W.config(5), 40, keep_truth=True)
+    n = np.diff(c5.hit_offsets.astype(np.int64))
+    assert n.min() >= 500 + 50 * 8 and n.max() <= 2000 + 400 * 12 + 4 * 12 * 12
+    assert 0 < sum(t["n_vertices"] > 0 for t in c5.truth) < 20
+    # slicing keeps CSR consistent; events are independent of how many are generated
+    s = c5.slice(3, 7)
+    assert s.n_events == 4 and s.hit_offsets[0] == 0 and np.array_equal(s.event(1)[1], c5.event(4)[1])
+    one = W.generate(W.config(5), 1, first_event=4)
+    assert np.array_equal(one.phi, c5.event(4)[1])
+
+
+def test_displaced_truth_geometry_is_self_consistent():
+    """The generator's displaced tracks really pass through their vertex: closest-approach parameters (d0, phi0)
+    reproduce the vertex position on the circle (pure geometry of the forward model, no voting arithmetic)."""
+    from paper_1309_6275_b200 import workloads as W
+    b = W.generate(W.config(2), keep_truth=True)
+    t = b.truth[0]
+    d0, phi0, kap = t["disp_d0"], t["disp_phi0"], t["disp_kappa"]
+    v = t["disp_vertex"]
+    vx = t["vertex_r"][v] * np.cos(t["vertex_phi"][v]); vy = t["vertex_r"][v] * np.sin(t["vertex_phi"][v])
+    cx = (1 / kap - d0) * -np.sin(phi0); cy = (1 / kap - d0) * np.cos(phi0)
+    assert np.allclose(np.hypot(vx - cx, vy - cy), 1 / np.abs(kap), rtol=1e-9)
+    assert np.all(np.abs(d0) <= t["vertex_r"][v] + 1e-9)
+
+
+_SHARD_SCRIPT = r'''
+import os, sys
+import numpy as np
+import torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+import bench
+rank = int(os.environ["RANK"]); world = int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+lo, hi = bench.shard_range(37, rank, world)
+mine = np.zeros(37, np.int64); mine[lo:hi] = 1
+import torch
+t = torch.from_numpy(mine); dist.all_reduce(t)
+assert t.tolist() == [1] * 37, t.tolist()                       # every event owned by exactly one rank
+ms = bench.max_over_ranks(10.0 + rank, dist)
+assert ms == 10.0 + world - 1
+tot = bench.sum_over_ranks(float(hi - lo), dist)
+assert tot == 37.0
+dist.destroy_process_group()
+print("shard ok", rank, lo, hi)
+'''
+
+
+def test_event_sharding_world_size_2_gloo(tmp_path):
+    script = tmp_path / "shard.py"
+    script.write_text(_SHARD_SCRIPT)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29611")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29611", str(script), ROOT],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("shard ok") == 2
