@@ -107,7 +107,8 @@ int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets,
  * written in ascending lin.
  *   d_peaks   [n_events][max_peaks_per_event]; only the first min(n_peaks[e], max_peaks) records are written
  *   d_n_peaks [n_events] u32: the TRUE number of peaks found (may exceed the capacity)
- * l_min must be in [1, n_layers].
+ * l_min must be in [1, n_layers].  Precondition: the planes are accumulators as hough_vote writes them, i.e.
+ * count[b] >= popcount(mask[b]) for every bin (a bin with count < l_min is rejected without reading its mask).
  */
 int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,
                 uint32_t l_min, hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream);
