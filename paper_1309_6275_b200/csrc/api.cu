@@ -114,6 +114,12 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         volatile float dd = d * d;                    // one fp32 multiply, kept out of any contraction
         d0c[id] = d; two_d0[id] = 2.0f * d; d0sq[id] = dd;
     }
+    // the branch-free exact division of the vote kernel is only used inside this range (vote.cu, div_rn_tame)
+    c->tame_tables = cfg->kappa_max >= 9.094947e-13f && cfg->kappa_max <= 1.0995116e12f;      // [2^-40, 2^40]
+    for (uint32_t id = 0; id < ND; ++id) {
+        const float a = fabsf(d0c[id]);
+        if (!(a == 0.f || (a >= 9.5367431640625e-07f && a <= 1048576.f))) c->tame_tables = false;
+    }
     c->kmax = cfg->kappa_max;
     c->inv_dk = (float)((double)NK / (2.0 * (double)cfg->kappa_max));
     c->nk_f = (float)NK;

@@ -8,7 +8,6 @@
 #include "hough.h"
 
 #define HOUGH_MAX_LAYERS 16
-#define HOUGH_TILE_W 32              // phi0 columns per vote tile = lanes of a warp
 
 // meta word of a prepared hit: bits 0..19 phi bucket pb (0 <= pb < NPHI), bits 20..23 layer,
 // bit 30 "wild" (r not a positive finite number: no window pruning), bit 31 "dropped" (never votes).
@@ -22,13 +21,13 @@
 struct Window { int lo1, hi1, lo2, hi2; };
 
 struct VotePlan {
-    int ids_per_tile;                // K: d0 bins per tile (1..4)
+    int tile_w;                      // W: phi0 columns per tile (8 in 3D, 32 in 2D)
+    int ids_per_tile;                // K: d0 bins per tile (1..6)
     int nk_tile;                     // kappa bins per tile (<= NK; NK split into nk_seg segments if it does not fit)
     int nk_seg;
     int threads;
-    int list_cap;                    // staged-hit list capacity (records)
     size_t smem_bytes;
-    int n_strips, n_tiles;           // ceil(ND/K), ceil(NPHI/32)
+    int n_strips, n_tiles;           // ceil(ND/K), ceil(NPHI/W)
 };
 
 struct PeakPlan {
@@ -46,6 +45,7 @@ struct hough_ctx {
     float* d_c0; float* d_s0;                 // [NPHI]
     float* d_d0c; float* d_two_d0; float* d_d0sq;   // [ND]
     float kmax, inv_dk, nk_f;
+    bool tame_tables;                         // d0 centres and kappa_max inside the range div_rn_tame is proven for
     // per-call workspace
     float4* d_rec;                            // [max_hits] {sin phi, cos phi, r, meta}
     uint32_t* d_meta;                         // [max_hits]
