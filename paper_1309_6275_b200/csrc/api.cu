@@ -37,7 +37,7 @@ void free_all(hough_ctx* c)
 {
     cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
     cudaFree(c->d_rec); cudaFree(c->d_meta); cudaFree(c->d_layer_r); cudaFree(c->d_win); cudaFree(c->d_status);
-    cudaFree(c->d_bitmap); cudaFree(c->d_rowcnt); cudaFree(c->d_jetkeys);
+    cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
     cudaFree(c->d_hp_jets); cudaFree(c->d_hp_npeaks); cudaFree(c->d_hp_njets); cudaFree(c->d_hp_flag);
@@ -133,7 +133,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS)); A(dev_alloc(&c->d_win, (size_t)HOUGH_MAX_LAYERS * ND));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
-    A(dev_alloc(&c->d_rowcnt, (size_t)cfg->max_events * ND * NP));
+    A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
     A(dev_alloc(&c->d_jetkeys, (size_t)cfg->max_events * cfg->max_peaks_per_event));
     if (cfg->host_chunk_events > 0) {
         const size_t E = cfg->max_events, H = cfg->max_hits;

@@ -31,11 +31,9 @@ struct VotePlan {
 };
 
 struct PeakPlan {
-    int tp;                          // phi0 rows per stencil tile
-    int qcap;                        // candidate-queue capacity per slab step
+    int unit_bins;                   // bins per lane-load of the stencil: 16 (256-bit) or 8 (128-bit)
+    int blocks_per_sm[2];            // resident blocks of the 128-bit / 256-bit kernel
     int threads;
-    size_t smem_bytes;
-    int n_tiles;
 };
 
 struct hough_ctx {
@@ -53,8 +51,8 @@ struct hough_ctx {
     uint32_t* d_layer_r;                      // [2*16] float bits: min r, max r per layer
     Window* d_win;                            // [16][ND]
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
-    uint8_t* d_bitmap;                        // [max_events][ND*NPHI][NK/8], rows defined where d_rowcnt > 0
-    uint16_t* d_rowcnt;                       // [max_events][ND*NPHI] peaks per row
+    uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
+    uint16_t* d_grpcnt;                       // [max_events][ceil(bins/256)] peaks per group of 256 / 512 bins
     uint64_t* d_jetkeys;                      // [max_events][max_peaks]
     // host path
     uint16_t* d_hp_count; uint16_t* d_hp_mask;     // [host_chunk_events][bins]

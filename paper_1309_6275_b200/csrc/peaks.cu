@@ -3,275 +3,202 @@
 // Definition (O-3; "looking for local maxima in the parameter space"): bin b is a peak
 // iff popcount(mask[b]) >= l_min and, for every existing neighbour n in the 3x3(x3) neighbourhood (phi0
 // periodic, kappa and d0 clipped), count[b] > count[n] or (count[b] == count[n] and lin(b) < lin(n)).
-// Because l_min >= 1 implies count[b] >= 1, a clipped neighbour is equivalent to a neighbour with count 0.
+// A peak therefore needs count[b] >= popcount(mask[b]) >= l_min >= 1.
 //
-// Stencil kernel.  A block owns TP phi0 rows x all kappa and marches along d0 with a ring of NSLOT count slabs
-// ((TP+2) rows with the phi0 halo, dense, no padding) in shared memory.  One thread fills the ring with 1-D
-// bulk async copies (cp.async.bulk ... mbarrier::complete_tx) NSLOT-3 slabs ahead, so every count byte is
-// pulled from HBM once (the halo rows come from L2) with no register staging.  Each step has two dense passes:
-//   pass 1  every thread reads 8 kappa bins per 128-bit shared load, rejects the vector if its packed maximum
-//           is below l_min (a peak needs count >= popcount(mask) >= l_min) and otherwise appends the bins with
-//           count >= l_min to a block queue;
-//   pass 2  one thread per queued bin runs the 8 / 26-neighbour test (same slab first, then the previous and
-//           the next slab only if some lane of the warp survived), and reads the mask plane only for bins that
-//           are local maxima.
-// The result is one bit per bin, written only for rows that hold a peak, plus a peak count per (d0, phi0) row.
-// Compaction kernel: one block per event scans the row counts in linear-index order (block prefix sum) and
-// writes the first max_peaks records; n_peaks is the true total.
+// Stencil kernel = one streaming pass over the count plane.  The plane of an event is cut, in linear-index
+// order, into units of UB bins (UB = 16: one 256-bit load per lane; UB = 8: one 128-bit load when the plane is
+// not a whole number of 32-byte units) and groups of 32 units (one warp-wide load: 1 KB or 512 B, contiguous).
+// A warp takes kUnroll consecutive groups per iteration, all loads issued before the first use, so that a
+// resident SM keeps 2048 threads x kUnroll x 32 B = 256 KB in flight: the pass is bound by HBM, not by
+// instruction issue (about 12 warp instructions per KB).  Per unit the packed
+// 16-bit maximum (VIMNMX3.U16x2) is compared with l_min; only bins with count >= l_min (rare at the trigger
+// thresholds) run the 8 / 26-neighbour test, whose neighbour reads go to L2 (the neighbouring rows and d0
+// slabs were streamed by neighbouring warps a moment earlier), and only local maxima read the mask plane.
+// Output: one bit per bin, written only for groups that hold a peak, and a peak count per group.
+// Compaction kernel: one block per event scans the group counts in linear-index order (block prefix sum,
+// 8 groups per thread) and writes the first max_peaks records; n_peaks is the true total.
 #include "hough_internal.cuh"
 
 namespace {
 
-// ---- mbarrier / bulk-copy primitives (PTX ISA: mbarrier, cp.async.bulk) ------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}"
-                 ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n\t}"
-        ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
+constexpr int kUnroll = 4;           // groups per warp iteration
+constexpr int kStencilThreads = 256;
 
 struct PeakParams {
     const uint16_t* count;
     const uint16_t* mask;
-    uint8_t* bitmap;             // [E][ND*NPHI][NK/8], a row is only defined where rowcnt > 0
-    uint16_t* rowcnt;            // [E][ND*NPHI] peaks per (d0, phi0) row (<= NK/2)
+    uint8_t* bitmap;             // [E][bins/8], a group's bytes are only defined where grpcnt > 0
+    uint16_t* grpcnt;            // [E][groups_per_event] peaks per group of 32*UB bins
     int n_d0, n_phi0, n_kappa;
-    int seg_len, n_seg, n_tiles;
+    uint32_t n_events;
+    uint32_t bins;               // per event
+    uint32_t units;              // per event = bins / UB
+    uint32_t groups;             // per event = ceil(units / 32)
+    uint32_t quads;              // per event = ceil(groups / kUnroll)
     uint32_t l_min;
-    int qcap;
 };
 
-// count of the bin at element offset o of a slab row, or of its left / right kappa neighbour (0 beyond the axis)
-__device__ __forceinline__ uint32_t max3_row(const uint16_t* row, int k, int NK)
+__device__ __forceinline__ void load_unit(const uint16_t* p, uint32_t (&r)[8])
 {
-    uint32_t m = row[k];
-    if (k > 0) m = max(m, (uint32_t)row[k - 1]);
-    if (k < NK - 1) m = max(m, (uint32_t)row[k + 1]);
-    return m;
+    asm volatile("ld.global.nc.L1::no_allocate.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "l"(p));
+}
+__device__ __forceinline__ void load_unit(const uint16_t* p, uint32_t (&r)[4])
+{
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "l"(p));
 }
 
-template <int TP, int NSLOT, int NT>
-__global__ void __launch_bounds__(NT) peak_stencil_kernel(const PeakParams p)
+__device__ __forceinline__ uint32_t packed_max(const uint32_t (&r)[8])
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int NK = p.n_kappa, N = p.n_phi0, ND = p.n_d0;
-    const int slab_elems = (TP + 2) * NK;
-    const int row_bytes = NK / 8;                                // bitmap bytes per row
-    uint16_t* slabs = reinterpret_cast<uint16_t*>(smem_raw);                                  // [NSLOT][(TP+2)*NK]
-    uint32_t* queue = reinterpret_cast<uint32_t*>(smem_raw + (size_t)NSLOT * slab_elems * 2);  // [qcap]
-    uint32_t* rowbits = queue + p.qcap;                                                         // [ceil(TP*NK/8 / 4)]
-    const int rowbits_words = (TP * row_bytes + 7) / 8 * 2;                                     // even: keeps bars 8-aligned
-    uint32_t* rowcnt_s = rowbits + rowbits_words;                                               // [TP]
-    uint32_t* q_n2 = rowcnt_s + TP;                                                             // [2] alternate by step
-    uint64_t* bars = reinterpret_cast<uint64_t*>(q_n2 + 2);                                     // [NSLOT]
-    const int tid = threadIdx.x;
+    const uint32_t a = __vimax3_u16x2(r[0], r[1], r[2]);
+    const uint32_t b = __vimax3_u16x2(r[3], r[4], r[5]);
+    return __vimax3_u16x2(__vimax3_u16x2(r[6], r[7], a), b, b);
+}
+__device__ __forceinline__ uint32_t packed_max(const uint32_t (&r)[4])
+{
+    return __vimax3_u16x2(__vimax3_u16x2(r[0], r[1], r[2]), r[3], r[3]);
+}
 
-    uint32_t b = blockIdx.x;
-    const int tile = b % p.n_tiles; b /= p.n_tiles;
-    const int seg = b % p.n_seg;
-    const uint32_t e = b / p.n_seg;
-    const int ip0 = tile * TP;
-    const int rows_valid = min(TP, N - ip0);                     // centre rows this block owns
-    const int id_a = seg * p.seg_len, id_b = min(ND, id_a + p.seg_len);
-    const int vec_per_row = NK / 8;
-    const size_t ev_bins = (size_t)ND * N * NK;
-    const size_t ev_rows = (size_t)ND * N;
-    const uint16_t* cnt_e = p.count + (size_t)e * ev_bins;
-    const uint16_t* msk_e = p.mask + (size_t)e * ev_bins;
-    uint8_t* bm_e = p.bitmap + (size_t)e * ev_rows * row_bytes;
-    uint16_t* rc_e = p.rowcnt + (size_t)e * ev_rows;
+__device__ __forceinline__ bool any_half_ge(uint32_t m, uint32_t l_min)
+{
+    return (m & 0xffffu) >= l_min || (m >> 16) >= l_min;
+}
 
-    if (tid == 0) {
-        for (int s = 0; s < NSLOT; ++s) mbar_init(&bars[s], 1);
-        q_n2[0] = 0; q_n2[1] = 0;
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+// O-3 for one bin with count c >= l_min at linear index lin of event planes cnt_e / msk_e.
+__device__ __noinline__ bool is_peak(const uint16_t* __restrict__ cnt_e, const uint16_t* __restrict__ msk_e,
+                                     uint32_t lin, uint32_t c, int ND, int N, int NK, uint32_t l_min)
+{
+    const uint32_t row = lin / (uint32_t)NK;
+    const int k = (int)(lin - row * (uint32_t)NK);
+    const int id = (int)(row / (uint32_t)N);
+    const int ip = (int)(row - (uint32_t)id * (uint32_t)N);
+    // same row: the left neighbour has the smaller linear index (must be strictly smaller), the right one may tie
+    if (k > 0 && (uint32_t)__ldg(cnt_e + lin - 1) >= c) return false;
+    if (k + 1 < NK && (uint32_t)__ldg(cnt_e + lin + 1) > c) return false;
+    const int k_lo = (k > 0) ? k - 1 : k, k_hi = (k + 1 < NK) ? k + 1 : k;
+#pragma unroll 1
+    for (int dd = 0; dd < 3; ++dd) {
+        const int idn = id + ((dd == 0) ? 0 : (dd == 1 ? -1 : 1));       // own d0 slab first
+        if (idn < 0 || idn >= ND) continue;
+#pragma unroll 1
+        for (int dp = -1; dp <= 1; ++dp) {
+            if (dd == 0 && dp == 0) continue;
+            int ipn = ip + dp;
+            if (ipn < 0) ipn += N;
+            if (ipn >= N) ipn -= N;
+            const uint32_t nrow = (uint32_t)idn * (uint32_t)N + (uint32_t)ipn;
+            const uint16_t* r = cnt_e + (size_t)nrow * NK;
+            // rows differ, so the order of the linear indices is the order of the rows (for every kappa offset)
+            const uint32_t bound = (nrow < row) ? c : c + 1u;            // neighbour must be < bound
+            for (int kn = k_lo; kn <= k_hi; ++kn)
+                if ((uint32_t)__ldg(r + kn) >= bound) return false;
+        }
     }
-    for (int i = tid; i < rowbits_words + TP; i += NT) rowbits[i] = 0;   // rowbits and rowcnt_s are contiguous
-    __syncthreads();
+    return (uint32_t)__popc((uint32_t)__ldg(msk_e + lin)) >= l_min;
+}
 
-    // slab `id` lives in slot (id - (id_a-1)) % NSLOT; its k-th use of the slot completes phase k
-    auto rel_of = [&](int id) { return id - (id_a - 1); };
-    auto issue_slab = [&](int id) {                              // thread 0 only
-        const int rel = rel_of(id);
-        uint64_t* bar = &bars[rel % NSLOT];
-        if (id < 0 || id >= ND) { mbar_arrive(bar); return; }    // nothing to load: just complete the phase
-        uint16_t* dst = slabs + (size_t)(rel % NSLOT) * slab_elems;
-        const uint16_t* src = cnt_e + (size_t)id * N * NK;
-        const int rows_needed = rows_valid + 2;                  // smem rows 0 .. rows_valid+1
-        mbar_arrive_expect_tx(bar, (uint32_t)rows_needed * NK * 2);
-        // smem row j holds global row (ip0 - 1 + j) mod N; merge runs of consecutive global rows
-        int j = 0;
-        while (j < rows_needed) {
-            int gr = (ip0 - 1 + j) % N; if (gr < 0) gr += N;
-            int run = min(rows_needed - j, N - gr);
-            bulk_g2s(dst + (size_t)j * NK, src + (size_t)gr * NK, (uint32_t)run * NK * 2, bar);
-            j += run;
-        }
-    };
+template <int UB>
+__global__ void __launch_bounds__(kStencilThreads) peak_stencil_kernel(const PeakParams p)
+{
+    constexpr int NW = UB / 2;                                   // 32-bit words per unit
+    const int lane = threadIdx.x & 31;
+    const uint32_t n_warps = gridDim.x * (kStencilThreads / 32);
+    const uint32_t gw = blockIdx.x * (kStencilThreads / 32) + (threadIdx.x >> 5);
+    const uint64_t total_quads = (uint64_t)p.n_events * p.quads;
 
-    constexpr int AHEAD = NSLOT - 3;                             // slabs in flight beyond id+1
-    if (tid == 0)
-        for (int id = id_a - 1; id <= id_a + 1 + AHEAD; ++id) issue_slab(id);
-
-    for (int id = id_a; id < id_b; ++id) {
-        // slabs id-1, id, id+1 must have landed (earlier phases of these barriers completed long ago)
-        if (id == id_a) {
-            mbar_wait(&bars[rel_of(id - 1) % NSLOT], (rel_of(id - 1) / NSLOT) & 1);
-            mbar_wait(&bars[rel_of(id) % NSLOT], (rel_of(id) / NSLOT) & 1);
-        }
-        mbar_wait(&bars[rel_of(id + 1) % NSLOT], (rel_of(id + 1) / NSLOT) & 1);
-        const uint16_t* s_prev = slabs + (size_t)(rel_of(id - 1) % NSLOT) * slab_elems;
-        const uint16_t* s_cur = slabs + (size_t)(rel_of(id) % NSLOT) * slab_elems;
-        const uint16_t* s_next = slabs + (size_t)(rel_of(id + 1) % NSLOT) * slab_elems;
-        const bool has_prev = id > 0, has_next = id + 1 < ND;
-        uint32_t* q_n = q_n2 + (id & 1);                         // reset two steps before its next use
-
-        // ---- pass 1: queue the bins with count >= l_min ----
-        const int n_vec = rows_valid * vec_per_row;
-        for (int t = tid; t < n_vec; t += NT) {
-            const int o = NK + t * 8;                            // element offset in the slab (row j+1 = centre row j)
-            const uint4 c8 = *reinterpret_cast<const uint4*>(s_cur + o);
-            const uint32_t m2 = __vmaxu2(__vmaxu2(c8.x, c8.y), __vmaxu2(c8.z, c8.w));
-            if (max(m2 & 0xffffu, m2 >> 16) >= p.l_min) {
-                const uint32_t w[4] = {c8.x, c8.y, c8.z, c8.w};
+    for (uint64_t q = gw; q < total_quads; q += n_warps) {
+        const uint32_t e = (uint32_t)(q / p.quads);
+        const uint32_t qi = (uint32_t)(q - (uint64_t)e * p.quads);
+        const uint16_t* cnt_e = p.count + (size_t)e * p.bins;
+        const uint32_t g0 = qi * kUnroll;
+        uint32_t d[kUnroll][NW];
 #pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    const uint32_t c = (w[q >> 1] >> ((q & 1) * 16)) & 0xffffu;
-                    if (c >= p.l_min) {
-                        const uint32_t slot = atomicAdd(q_n, 1u);
-                        if (slot < (uint32_t)p.qcap) queue[slot] = (uint32_t)(o + q);
-                    }
+        for (int u = 0; u < kUnroll; ++u) {
+            const uint32_t unit = (g0 + u) * 32u + lane;
+            if (unit < p.units) load_unit(cnt_e + (size_t)unit * UB, d[u]);
+            else {
+#pragma unroll
+                for (int w = 0; w < NW; ++w) d[u][w] = 0;
+            }
+        }
+        uint32_t m = packed_max(d[0]);
+#pragma unroll
+        for (int u = 1; u < kUnroll; ++u) { const uint32_t t = packed_max(d[u]); m = __vimax3_u16x2(m, t, t); }
+        const bool ge = any_half_ge(m, p.l_min);
+        uint32_t bits[kUnroll];
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) bits[u] = 0;
+        if (ge) {                                                // rare: some bin of this lane may be a peak
+            const uint16_t* msk_e = p.mask + (size_t)e * p.bins;
+#pragma unroll
+            for (int u = 0; u < kUnroll; ++u) {
+                if (!any_half_ge(packed_max(d[u]), p.l_min)) continue;
+                const uint32_t lin0 = ((g0 + u) * 32u + lane) * UB;
+#pragma unroll
+                for (int j = 0; j < UB; ++j) {
+                    const uint32_t c = (d[u][j >> 1] >> ((j & 1) * 16)) & 0xffffu;
+                    if (c >= p.l_min && is_peak(cnt_e, msk_e, lin0 + j, c, p.n_d0, p.n_phi0, p.n_kappa, p.l_min))
+                        bits[u] |= 1u << j;
                 }
             }
         }
-        __syncthreads();
-        const uint32_t n_q = *q_n;
-        const bool overflow = n_q > (uint32_t)p.qcap;            // stress case: walk every bin instead of the queue
-        const uint32_t n_items = overflow ? (uint32_t)(rows_valid * NK) : n_q;
-
-        // ---- pass 2: full neighbourhood test of the queued bins ----
-        for (uint32_t base = 0; base < n_items; base += NT) {
-            const uint32_t t = base + tid;
-            bool ok = false;
-            int o = 0, k = 0, j = 0;
-            uint32_t c = 0;
-            if (t < n_items) {
-                o = overflow ? (int)(NK + t) : (int)queue[t];
-                j = o / NK - 1; k = o - (j + 1) * NK;
-                c = s_cur[o];
-                ok = c >= p.l_min;
-            }
-            if (ok) {
-                const int ip = ip0 + j;
-                // neighbours with a smaller linear index must be strictly smaller, the others may tie
-                const uint32_t left = (k > 0) ? (uint32_t)s_cur[o - 1] : 0u;
-                const uint32_t right = (k < NK - 1) ? (uint32_t)s_cur[o + 1] : 0u;
-                ok = (left < c) && (right <= c);
-                if (ok) {
-                    const uint32_t up = max3_row(s_cur + o - k - NK, k, NK), dn = max3_row(s_cur + o - k + NK, k, NK);
-                    ok = ((ip == 0) ? (up <= c) : (up < c)) &&           // row ip-1 wraps to NPHI-1 > ip
-                         ((ip == N - 1) ? (dn < c) : (dn <= c));         // row ip+1 wraps to 0 < ip
+        uint16_t* gc = p.grpcnt + (size_t)e * p.groups;
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+            const uint32_t g = g0 + u;
+            if (g >= p.groups) break;                            // warp-uniform
+            const unsigned any = __ballot_sync(0xffffffffu, bits[u] != 0);
+            uint32_t n = 0;
+            if (any) {                                           // warp-uniform
+                n = __reduce_add_sync(0xffffffffu, (uint32_t)__popc(bits[u]));
+                const uint32_t unit = g * 32u + lane;
+                if (unit < p.units) {
+                    uint8_t* bm = p.bitmap + (size_t)e * (p.bins / 8) + (size_t)unit * (UB / 8);
+                    if (UB == 16) *reinterpret_cast<uint16_t*>(bm) = (uint16_t)bits[u];
+                    else *bm = (uint8_t)bits[u];
                 }
             }
-            if (__any_sync(0xffffffffu, ok)) {
-                if (ok && has_prev) {
-                    const uint16_t* r0 = s_prev + o - k;
-                    const uint32_t m = max(max(max3_row(r0 - NK, k, NK), max3_row(r0, k, NK)), max3_row(r0 + NK, k, NK));
-                    ok = m < c;
-                }
-                if (ok && has_next) {
-                    const uint16_t* r0 = s_next + o - k;
-                    const uint32_t m = max(max(max3_row(r0 - NK, k, NK), max3_row(r0, k, NK)), max3_row(r0 + NK, k, NK));
-                    ok = m <= c;
-                }
-                if (ok) {
-                    const size_t lin = ((size_t)id * N + (ip0 + j)) * NK + k;
-                    if ((uint32_t)__popc((uint32_t)__ldg(msk_e + lin)) >= p.l_min) {
-                        const int byte = j * row_bytes + (k >> 3);
-                        atomicOr(&rowbits[byte >> 2], (1u << (k & 7)) << ((byte & 3) * 8));
-                        atomicAdd(&rowcnt_s[j], 1u);
-                    }
-                }
-            }
-        }
-        __syncthreads();                                         // slab id-1 is free; rowbits / rowcnt_s complete
-
-        if (tid == 0) {
-            issue_slab(id + 2 + AHEAD);
-            *q_n = 0;
-        }
-        // ---- write the row counts, and the bitmap rows that hold a peak ----
-        const size_t row0 = (size_t)id * N + ip0;
-        if (tid < rows_valid) rc_e[row0 + tid] = (uint16_t)rowcnt_s[tid];
-        bool dirty = false;
-        for (int j = 0; j < rows_valid; ++j) {
-            if (rowcnt_s[j] == 0) continue;                      // block-uniform
-            dirty = true;
-            const uint8_t* srcb = reinterpret_cast<const uint8_t*>(rowbits) + (size_t)j * row_bytes;
-            uint8_t* dstb = bm_e + (row0 + j) * row_bytes;
-            for (int i = tid; i < row_bytes; i += NT) dstb[i] = srcb[i];
-        }
-        if (dirty) {                                             // block-uniform
-            __syncthreads();
-            for (int i = tid; i < rowbits_words + TP; i += NT) rowbits[i] = 0;
-            // ordered before the next pass 2 by the next step's barrier after pass 1
+            if (lane == 0) gc[g] = (uint16_t)n;
         }
     }
-    // drain the copies still in flight before the block (and its shared memory) goes away
-    if (tid == 0)
-        for (int id = id_b + 1; id <= id_b + 1 + AHEAD; ++id) mbar_wait(&bars[rel_of(id) % NSLOT], (rel_of(id) / NSLOT) & 1);
 }
 
-// ---- A4: ordered compaction from the row counts + bitmap rows ----------------------------------------------
+// ---- A4: ordered compaction from the group counts + bitmap --------------------------------------------------
 
-__global__ void __launch_bounds__(1024) peak_compact_kernel(const uint16_t* __restrict__ count,
-                                                            const uint16_t* __restrict__ mask,
-                                                            const uint8_t* __restrict__ bitmap,
-                                                            const uint16_t* __restrict__ rowcnt, int n_rows,
-                                                            int n_kappa, uint32_t max_peaks,
-                                                            hough_peak* __restrict__ peaks,
-                                                            uint32_t* __restrict__ n_peaks)
+constexpr int kCompactThreads = 1024;
+constexpr int kGroupsPerThread = 8;
+
+__global__ void __launch_bounds__(kCompactThreads) peak_compact_kernel(const uint16_t* __restrict__ count,
+                                                                       const uint16_t* __restrict__ mask,
+                                                                       const uint8_t* __restrict__ bitmap,
+                                                                       const uint16_t* __restrict__ grpcnt,
+                                                                       uint32_t bins, uint32_t groups,
+                                                                       uint32_t group_bins, uint32_t max_peaks,
+                                                                       hough_peak* __restrict__ peaks,
+                                                                       uint32_t* __restrict__ n_peaks)
 {
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_total;
     const uint32_t e = blockIdx.x;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int row_bytes = n_kappa / 8;
-    const size_t ev_bins = (size_t)n_rows * n_kappa;
-    const uint8_t* bm = bitmap + (size_t)e * n_rows * row_bytes;
-    const uint16_t* rc = rowcnt + (size_t)e * n_rows;
-    const uint16_t* cnt_e = count + (size_t)e * ev_bins;
-    const uint16_t* msk_e = mask + (size_t)e * ev_bins;
+    const uint8_t* bm = bitmap + (size_t)e * (bins / 8);
+    const uint16_t* gc = grpcnt + (size_t)e * groups;
+    const uint16_t* cnt_e = count + (size_t)e * bins;
+    const uint16_t* msk_e = mask + (size_t)e * bins;
     hough_peak* out = peaks + (size_t)e * max_peaks;
+    const uint32_t group_bytes = group_bins / 8;
     uint32_t running = 0;
-    for (int base = 0; base < n_rows; base += 1024) {
-        const int row = base + tid;
-        const uint32_t c = (row < n_rows) ? (uint32_t)rc[row] : 0u;
+    for (uint32_t base = 0; base < groups; base += kCompactThreads * kGroupsPerThread) {
+        const uint32_t g_first = base + (uint32_t)tid * kGroupsPerThread;
+        uint32_t cg[kGroupsPerThread];
+        uint32_t c = 0;
+#pragma unroll
+        for (int i = 0; i < kGroupsPerThread; ++i) {
+            cg[i] = (g_first + i < groups) ? (uint32_t)gc[g_first + i] : 0u;
+            c += cg[i];
+        }
         // block exclusive prefix sum of c
         uint32_t incl = c;
 #pragma unroll
@@ -294,16 +221,22 @@ __global__ void __launch_bounds__(1024) peak_compact_kernel(const uint16_t* __re
         __syncthreads();
         uint32_t pos = running + s_warp[warp] + incl - c;
         if (c > 0 && pos < max_peaks) {
-            const uint8_t* rp = bm + (size_t)row * row_bytes;
-            for (int i = 0; i < row_bytes && pos < max_peaks; ++i) {
-                uint32_t byte = rp[i];
-                while (byte && pos < max_peaks) {
-                    const int q = __ffs(byte) - 1;
-                    byte &= byte - 1;
-                    const size_t lin = (size_t)row * n_kappa + i * 8 + q;
-                    hough_peak pk;
-                    pk.lin = (uint32_t)lin; pk.count = cnt_e[lin]; pk.mask = msk_e[lin];
-                    out[pos++] = pk;
+            for (int i = 0; i < kGroupsPerThread && pos < max_peaks; ++i) {
+                if (cg[i] == 0) continue;
+                const uint32_t g = g_first + i;
+                const uint8_t* gp = bm + (size_t)g * group_bytes;
+                const uint32_t lin_g = g * group_bins;
+                const uint32_t nbytes = min(group_bytes, bins / 8 - g * group_bytes);     // ragged last group
+                for (uint32_t b = 0; b < nbytes && pos < max_peaks; ++b) {
+                    uint32_t byte = gp[b];
+                    while (byte && pos < max_peaks) {
+                        const int qb = __ffs(byte) - 1;
+                        byte &= byte - 1;
+                        const uint32_t lin = lin_g + b * 8 + qb;
+                        hough_peak pk;
+                        pk.lin = lin; pk.count = cnt_e[lin]; pk.mask = msk_e[lin];
+                        out[pos++] = pk;
+                    }
                 }
             }
         }
@@ -313,45 +246,19 @@ __global__ void __launch_bounds__(1024) peak_compact_kernel(const uint16_t* __re
     if (tid == 0) n_peaks[e] = running;
 }
 
-constexpr int kSlots = 5;
-constexpr int kStencilThreads = 256;
-
-size_t stencil_smem_bytes(int tp, int nk, int qcap)
-{
-    const size_t slabs = (size_t)kSlots * (tp + 2) * nk * 2;
-    const size_t rowbits_words = ((size_t)tp * (nk / 8) + 7) / 8 * 2;
-    return slabs + (size_t)qcap * 4 + rowbits_words * 4 + (size_t)tp * 4 + 8 + (size_t)kSlots * 8;
-}
-
-template <int TP>
-cudaError_t launch_stencil(const PeakParams& p, uint32_t nb, size_t smem, cudaStream_t st)
-{
-    auto kern = peak_stencil_kernel<TP, kSlots, kStencilThreads>;
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return err;
-    kern<<<nb, kStencilThreads, smem, st>>>(p);
-    return cudaGetLastError();
-}
-
 }  // namespace
 
 cudaError_t plan_peaks(hough_ctx* c)
 {
     PeakPlan& pp = c->peak;
-    const int nk = (int)c->cfg.n_kappa;
+    const uint64_t bins = (uint64_t)c->cfg.n_d0 * c->cfg.n_phi0 * c->cfg.n_kappa;
     pp.threads = kStencilThreads;
-    // largest tile height whose ring fits twice on an SM (else once)
-    const int cand[4] = {16, 8, 4, 2};
-    pp.tp = 0;
-    for (int pass = 0; pass < 2 && pp.tp == 0; ++pass)
-        for (int i = 0; i < 4; ++i) {
-            const int qcap = 2 * nk > 2048 ? 2048 : 2 * nk;
-            const size_t s = stencil_smem_bytes(cand[i], nk, qcap);
-            if (s <= (pass == 0 ? 112u * 1024u : 226u * 1024u)) { pp.tp = cand[i]; pp.qcap = qcap; pp.smem_bytes = s; break; }
-        }
-    if (pp.tp == 0) return cudaErrorInvalidConfiguration;
-    pp.n_tiles = (int)((c->cfg.n_phi0 + pp.tp - 1) / pp.tp);
-    return cudaSuccess;
+    pp.unit_bins = (bins % 16 == 0) ? 16 : 8;                    // n_kappa % 8 == 0 is a hough_create precondition
+    cudaError_t err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pp.blocks_per_sm[0], peak_stencil_kernel<8>,
+                                                                    kStencilThreads, 0);
+    if (err != cudaSuccess) return err;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&pp.blocks_per_sm[1], peak_stencil_kernel<16>,
+                                                         kStencilThreads, 0);
 }
 
 cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,
@@ -360,33 +267,29 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
     if (n_events == 0) return cudaSuccess;
     const PeakPlan& pp = c->peak;
     PeakParams p;
-    p.count = d_count; p.mask = d_mask; p.bitmap = c->d_bitmap; p.rowcnt = c->d_rowcnt;
+    p.count = d_count; p.mask = d_mask; p.bitmap = c->d_bitmap; p.grpcnt = c->d_grpcnt;
     p.n_d0 = (int)c->cfg.n_d0; p.n_phi0 = (int)c->cfg.n_phi0; p.n_kappa = (int)c->cfg.n_kappa;
-    p.n_tiles = pp.n_tiles; p.l_min = l_min; p.qcap = pp.qcap;
-    // split d0 into segments only when there are too few blocks to fill the machine
-    int n_seg = 1;
-    const uint64_t base_blocks = (uint64_t)n_events * pp.n_tiles;
-    const uint64_t want = (uint64_t)c->sm_count * 4;
-    if (base_blocks < want && p.n_d0 >= 8) {
-        n_seg = (int)((want + base_blocks - 1) / base_blocks);
-        if (n_seg > p.n_d0 / 4) n_seg = p.n_d0 / 4;
-        if (n_seg < 1) n_seg = 1;
-    }
-    p.seg_len = (p.n_d0 + n_seg - 1) / n_seg;
-    p.n_seg = (p.n_d0 + p.seg_len - 1) / p.seg_len;
-    const uint64_t nb = base_blocks * p.n_seg;
-    if (nb > 0x7fffffffull) return cudaErrorInvalidConfiguration;
-    cudaError_t err;
-    switch (pp.tp) {
-        case 16: err = launch_stencil<16>(p, (uint32_t)nb, pp.smem_bytes, st); break;
-        case 8: err = launch_stencil<8>(p, (uint32_t)nb, pp.smem_bytes, st); break;
-        case 4: err = launch_stencil<4>(p, (uint32_t)nb, pp.smem_bytes, st); break;
-        default: err = launch_stencil<2>(p, (uint32_t)nb, pp.smem_bytes, st); break;
-    }
+    p.n_events = n_events; p.l_min = l_min;
+    p.bins = (uint32_t)((uint64_t)c->cfg.n_d0 * c->cfg.n_phi0 * c->cfg.n_kappa);
+    // 256-bit loads need 32-byte aligned units: every event plane starts at a multiple of 32 bytes iff the
+    // caller's base pointer does and bins % 16 == 0
+    const int ub = (pp.unit_bins == 16 && (((uintptr_t)d_count) & 31u) == 0) ? 16 : 8;
+    p.units = p.bins / (uint32_t)ub;
+    p.groups = (p.units + 31u) / 32u;
+    p.quads = (p.groups + kUnroll - 1) / kUnroll;
+    const uint64_t total_quads = (uint64_t)n_events * p.quads;
+    const uint64_t warps_wanted = total_quads;
+    uint64_t nb = (warps_wanted + (kStencilThreads / 32) - 1) / (kStencilThreads / 32);
+    const uint64_t cap = (uint64_t)c->sm_count * pp.blocks_per_sm[ub == 16];    // one resident wave
+    if (nb > cap) nb = cap;
+    if (ub == 16) peak_stencil_kernel<16><<<(unsigned)nb, kStencilThreads, 0, st>>>(p);
+    else peak_stencil_kernel<8><<<(unsigned)nb, kStencilThreads, 0, st>>>(p);
     ++c->launches;
+    cudaError_t err = cudaGetLastError();
     if (err != cudaSuccess) return err;
-    peak_compact_kernel<<<n_events, 1024, 0, st>>>(d_count, d_mask, c->d_bitmap, c->d_rowcnt, p.n_d0 * p.n_phi0,
-                                                   p.n_kappa, c->cfg.max_peaks_per_event, d_peaks, d_n_peaks);
+    peak_compact_kernel<<<n_events, kCompactThreads, 0, st>>>(d_count, d_mask, c->d_bitmap, c->d_grpcnt, p.bins,
+                                                              p.groups, 32u * (uint32_t)ub,
+                                                              c->cfg.max_peaks_per_event, d_peaks, d_n_peaks);
     ++c->launches;
     return cudaGetLastError();
 }
