@@ -21,7 +21,13 @@
 
 namespace {
 
-constexpr int kUnroll = 4;           // groups per warp iteration
+#ifndef STENCIL_UNROLL
+#define STENCIL_UNROLL 4
+#endif
+#ifndef STENCIL_MINB
+#define STENCIL_MINB 3
+#endif
+constexpr int kUnroll = STENCIL_UNROLL;           // groups per warp iteration
 constexpr int kStencilThreads = 256;
 
 struct PeakParams {
@@ -36,6 +42,7 @@ struct PeakParams {
     uint32_t groups;             // per event = ceil(units / 32)
     uint32_t quads;              // per event = ceil(groups / kUnroll)
     uint32_t l_min;
+    uint32_t row_aligned;        // n_kappa % UB == 0: a unit never straddles two kappa rows
 };
 
 __device__ __forceinline__ void load_unit(const uint16_t* p, uint32_t (&r)[8])
@@ -66,7 +73,10 @@ __device__ __forceinline__ bool any_half_ge(uint32_t m, uint32_t l_min)
     return (m & 0xffffu) >= l_min || (m >> 16) >= l_min;
 }
 
-// O-3 for one bin with count c >= l_min at linear index lin of event planes cnt_e / msk_e.
+// O-3 for one bin with count c >= l_min at linear index lin of event planes cnt_e / msk_e.  Three batches of
+// loads, each issued before its first comparison: the kappa neighbours, the two phi0 rows of the own d0 slab
+// (hot in L2: streamed by the neighbouring warps), then the six rows of the slabs id-1 / id+1.  A clipped
+// neighbour reads as 0, which never beats c >= 1.
 __device__ __noinline__ bool is_peak(const uint16_t* __restrict__ cnt_e, const uint16_t* __restrict__ msk_e,
                                      uint32_t lin, uint32_t c, int ND, int N, int NK, uint32_t l_min)
 {
@@ -74,33 +84,52 @@ __device__ __noinline__ bool is_peak(const uint16_t* __restrict__ cnt_e, const u
     const int k = (int)(lin - row * (uint32_t)NK);
     const int id = (int)(row / (uint32_t)N);
     const int ip = (int)(row - (uint32_t)id * (uint32_t)N);
+    const bool has_l = k > 0, has_r = k + 1 < NK;
     // same row: the left neighbour has the smaller linear index (must be strictly smaller), the right one may tie
-    if (k > 0 && (uint32_t)__ldg(cnt_e + lin - 1) >= c) return false;
-    if (k + 1 < NK && (uint32_t)__ldg(cnt_e + lin + 1) > c) return false;
-    const int k_lo = (k > 0) ? k - 1 : k, k_hi = (k + 1 < NK) ? k + 1 : k;
-#pragma unroll 1
-    for (int dd = 0; dd < 3; ++dd) {
-        const int idn = id + ((dd == 0) ? 0 : (dd == 1 ? -1 : 1));       // own d0 slab first
-        if (idn < 0 || idn >= ND) continue;
-#pragma unroll 1
-        for (int dp = -1; dp <= 1; ++dp) {
-            if (dd == 0 && dp == 0) continue;
-            int ipn = ip + dp;
-            if (ipn < 0) ipn += N;
-            if (ipn >= N) ipn -= N;
-            const uint32_t nrow = (uint32_t)idn * (uint32_t)N + (uint32_t)ipn;
-            const uint16_t* r = cnt_e + (size_t)nrow * NK;
-            // rows differ, so the order of the linear indices is the order of the rows (for every kappa offset)
-            const uint32_t bound = (nrow < row) ? c : c + 1u;            // neighbour must be < bound
-            for (int kn = k_lo; kn <= k_hi; ++kn)
-                if ((uint32_t)__ldg(r + kn) >= bound) return false;
-        }
-    }
+    const uint32_t vl = has_l ? (uint32_t)__ldg(cnt_e + lin - 1) : 0u;
+    const uint32_t vr = has_r ? (uint32_t)__ldg(cnt_e + lin + 1) : 0u;
+    if (!(vl < c && vr <= c)) return false;
+    const int ipm = (ip == 0) ? N - 1 : ip - 1, ipp = (ip == N - 1) ? 0 : ip + 1;
+    // max over the three kappa offsets of row nrow must be < c if that row precedes ours in linear-index
+    // order, <= c otherwise (rows differ, so the order of the indices is the order of the rows)
+    auto row_ok = [&](uint32_t nrow, bool ok) {
+        const uint16_t* r = cnt_e + (size_t)nrow * NK + k;
+        const uint32_t v0 = (ok && has_l) ? (uint32_t)__ldg(r - 1) : 0u;
+        const uint32_t v1 = ok ? (uint32_t)__ldg(r) : 0u;
+        const uint32_t v2 = (ok && has_r) ? (uint32_t)__ldg(r + 1) : 0u;
+        return max(max(v0, v1), v2) < ((nrow < row) ? c : c + 1u);
+    };
+    const uint32_t base = (uint32_t)id * (uint32_t)N;
+    const bool a0 = row_ok(base + (uint32_t)ipm, true), a1 = row_ok(base + (uint32_t)ipp, true);
+    if (!(a0 && a1)) return false;
+    const bool dn = id > 0, up = id + 1 < ND;
+    const uint32_t bd = dn ? base - (uint32_t)N : base, bu = up ? base + (uint32_t)N : base;
+    const bool b0 = row_ok(bd + (uint32_t)ipm, dn), b1 = row_ok(bd + (uint32_t)ip, dn), b2 = row_ok(bd + (uint32_t)ipp, dn);
+    const bool c0 = row_ok(bu + (uint32_t)ipm, up), c1 = row_ok(bu + (uint32_t)ip, up), c2 = row_ok(bu + (uint32_t)ipp, up);
+    if (!(b0 && b1 && b2 && c0 && c1 && c2)) return false;
     return (uint32_t)__popc((uint32_t)__ldg(msk_e + lin)) >= l_min;
 }
 
+// Bins of one unit with count >= l_min that are not beaten by a neighbour INSIDE the unit (left must be strictly
+// smaller, right may tie).  Only valid when a unit never straddles two kappa rows (n_kappa % UB == 0).
+template <int NW>
+__device__ __forceinline__ uint32_t unit_candidates(const uint32_t (&d)[NW], uint32_t l_min, bool row_aligned)
+{
+    uint32_t bits = 0;
+    uint32_t prev = 0;
+#pragma unroll
+    for (int j = 0; j < 2 * NW; ++j) {
+        const uint32_t c = (d[j >> 1] >> ((j & 1) * 16)) & 0xffffu;
+        const uint32_t next = (j + 1 < 2 * NW) ? ((d[(j + 1) >> 1] >> (((j + 1) & 1) * 16)) & 0xffffu) : 0u;
+        const bool inside = !row_aligned || (prev < c && next <= c);
+        if (c >= l_min && inside) bits |= 1u << j;
+        prev = c;
+    }
+    return bits;
+}
+
 template <int UB>
-__global__ void __launch_bounds__(kStencilThreads) peak_stencil_kernel(const PeakParams p)
+__global__ void __launch_bounds__(kStencilThreads, STENCIL_MINB) peak_stencil_kernel(const PeakParams p)
 {
     constexpr int NW = UB / 2;                                   // 32-bit words per unit
     const int lane = threadIdx.x & 31;
@@ -136,11 +165,12 @@ __global__ void __launch_bounds__(kStencilThreads) peak_stencil_kernel(const Pea
             for (int u = 0; u < kUnroll; ++u) {
                 if (!any_half_ge(packed_max(d[u]), p.l_min)) continue;
                 const uint32_t lin0 = ((g0 + u) * 32u + lane) * UB;
-#pragma unroll
-                for (int j = 0; j < UB; ++j) {
-                    const uint32_t c = (d[u][j >> 1] >> ((j & 1) * 16)) & 0xffffu;
-                    if (c >= p.l_min && is_peak(cnt_e, msk_e, lin0 + j, c, p.n_d0, p.n_phi0, p.n_kappa, p.l_min))
-                        bits[u] |= 1u << j;
+                uint32_t cand = unit_candidates<NW>(d[u], p.l_min, p.row_aligned != 0);
+                while (cand) {
+                    const int j = __ffs(cand) - 1;
+                    cand &= cand - 1;
+                    const uint32_t c = (uint32_t)__ldg(cnt_e + lin0 + j);       // re-read: no dynamic register indexing
+                    if (is_peak(cnt_e, msk_e, lin0 + j, c, p.n_d0, p.n_phi0, p.n_kappa, p.l_min)) bits[u] |= 1u << j;
                 }
             }
         }
@@ -274,6 +304,7 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
     // 256-bit loads need 32-byte aligned units: every event plane starts at a multiple of 32 bytes iff the
     // caller's base pointer does and bins % 16 == 0
     const int ub = (pp.unit_bins == 16 && (((uintptr_t)d_count) & 31u) == 0) ? 16 : 8;
+    p.row_aligned = (c->cfg.n_kappa % (uint32_t)ub == 0) ? 1u : 0u;
     p.units = p.bins / (uint32_t)ub;
     p.groups = (p.units + 31u) / 32u;
     p.quads = (p.groups + kUnroll - 1) / kUnroll;
