@@ -36,7 +36,8 @@ cudaError_t dev_alloc(T** p, size_t n)
 void free_all(hough_ctx* c)
 {
     cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
-    cudaFree(c->d_rec); cudaFree(c->d_meta); cudaFree(c->d_layer_r); cudaFree(c->d_win); cudaFree(c->d_status);
+    cudaFree(c->d_rec); cudaFree(c->d_rec_u); cudaFree(c->d_key); cudaFree(c->d_seg); cudaFree(c->d_btab);
+    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
@@ -129,8 +130,11 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     auto A = [&](cudaError_t e2) { if (err == cudaSuccess) err = e2; };
     A(dev_alloc(&c->d_c0, NP)); A(dev_alloc(&c->d_s0, NP));
     A(dev_alloc(&c->d_d0c, ND)); A(dev_alloc(&c->d_two_d0, ND)); A(dev_alloc(&c->d_d0sq, ND));
-    A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_meta, cfg->max_hits));
-    A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS)); A(dev_alloc(&c->d_win, (size_t)HOUGH_MAX_LAYERS * ND));
+    A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_rec_u, cfg->max_hits)); A(dev_alloc(&c->d_key, cfg->max_hits));
+    A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
+    A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
+    A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS));
+    A(dev_alloc(&c->d_tilewin, (size_t)HOUGH_MAX_LAYERS * c->vote.n_strips));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
     A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
@@ -194,7 +198,7 @@ int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets,
     ctx->last_stream = st;
     if (n_events == 0) return HOUGH_OK;
     CK(launch_prep(ctx, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, st), "hit preparation");
-    CK(launch_vote(ctx, n_events, d_hit_offsets, d_hit_offsets, d_count, d_mask, st), "vote kernel");
+    CK(launch_vote(ctx, 0, n_events, d_count, d_mask, st), "vote kernel");
     return HOUGH_OK;
 }
 
@@ -262,7 +266,7 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
         cudaEvent_t t[4] = {nullptr, nullptr, nullptr, nullptr};
         if (ms_stage) for (int i = 0; i < 4; ++i) { CK(cudaEventCreate(&t[i]), "event"); evs.push_back(t[i]); }
         if (ms_stage) cudaEventRecord(t[0], st);
-        CK(launch_vote(ctx, ne, ctx->d_hp_off + e0, ctx->d_hp_off, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel");
+        CK(launch_vote(ctx, e0, ne, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel");
         if (ms_stage) cudaEventRecord(t[1], st);
         CK(launch_peaks(ctx, ne, ctx->d_hp_count, ctx->d_hp_mask, l_min, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event,
                         ctx->d_hp_npeaks + e0, st), "peak kernels");

@@ -9,20 +9,23 @@
 
 #define HOUGH_MAX_LAYERS 16
 
-// meta word of a prepared hit: bits 0..19 phi bucket pb (0 <= pb < NPHI), bits 20..23 layer,
-// bit 30 "wild" (r not a positive finite number: no window pruning), bit 31 "dropped" (never votes).
-#define META_PB_MASK 0xFFFFFu
-#define META_LAYER_SHIFT 20
-#define META_WILD (1u << 30)
-#define META_DROP (1u << 31)
+// Prepared hit record (float4): {RN32(sin phi), RN32(cos phi), r, bits}, bits = (0x10000 << layer) | wild, where
+// "wild" marks a hit whose r is outside [2^-20, 2^20] or not finite (no window pruning, generic IEEE division).
 
-// pruning window of (layer, id): columns ip that can receive a vote from a hit in phi bucket pb satisfy
-// ip - pb in [lo1, hi1] or [lo2, hi2] (mod NPHI).  lo > hi encodes "empty".
-struct Window { int lo1, hi1, lo2, hi2; };
+// Hits that can reach a tile starting at phi0 column ip0, for one (layer, d0 strip): the hit's own phi0 column
+// pb lies in [ip0 + a_i, ip0 + a_i + len_i) mod NPHI for i = 0 or 1.  len <= 0: no run; len >= NPHI: every hit.
+struct TileWin { int a0, len0, a1, len1; };
+
+// per event: start of the 16 layer segments and of the wild segment in the sorted records, then the end
+constexpr int kSegStride = HOUGH_MAX_LAYERS + 2;
 
 struct VotePlan {
-    int tile_w;                      // W: phi0 columns per tile (8 in 3D, 32 in 2D)
-    int ids_per_tile;                // K: d0 bins per tile (1..6)
+    int k_lane;                      // KL: rows per lane; a tile has 32 * KL rows
+    int tile_w;                      // phi0 columns per tile (8 in 3D, 32 * KL in 2D)
+    int ids_per_tile;                // d0 bins per tile (4 * KL in 3D, 1 in 2D)
+    int sh;                          // phi bucket of the hit sort = phi0 column >> sh
+    uint32_t nb;                     // phi buckets per layer
+    uint32_t stage_hits;             // records per stage of the hit ring
     int nk_tile;                     // kappa bins per tile (<= NK; NK split into nk_seg segments if it does not fit)
     int nk_seg;
     int threads;
@@ -46,10 +49,13 @@ struct hough_ctx {
     float kmax, inv_dk, nk_f;
     bool tame_tables;                         // d0 centres and kappa_max inside the range div_rn_tame is proven for
     // per-call workspace
-    float4* d_rec;                            // [max_hits] {sin phi, cos phi, r, meta}
-    uint32_t* d_meta;                         // [max_hits]
+    float4* d_rec_u;                          // [max_hits] prepared hits in input order (sort scratch)
+    uint32_t* d_key;                          // [max_hits] sort keys (sort scratch)
+    float4* d_rec;                            // [max_hits] prepared hits sorted per event by (layer, phi bucket)
+    uint32_t* d_seg;                          // [max_events][kSegStride]
+    uint16_t* d_btab;                         // [max_events][16][nb + 1] bucket starts relative to the layer segment
     uint32_t* d_layer_r;                      // [2*16] float bits: min r, max r per layer
-    Window* d_win;                            // [16][ND]
+    TileWin* d_tilewin;                       // [16][n_strips]
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
     uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
     uint16_t* d_grpcnt;                       // [max_events][ceil(bins/256)] peaks per group of 256 / 512 bins
@@ -70,8 +76,8 @@ struct hough_ctx {
 // launchers (each returns a cudaError_t from the launch; all asynchronous on `st`)
 cudaError_t launch_prep(hough_ctx* c, uint32_t n_events, const uint32_t* d_off, uint64_t n_hits,
                         const float* d_r, const float* d_phi, const uint8_t* d_layer, cudaStream_t st);
-cudaError_t launch_vote(hough_ctx* c, uint32_t n_events, const uint32_t* d_off, const uint32_t* d_base,
-                        uint16_t* d_count, uint16_t* d_mask, cudaStream_t st);
+cudaError_t launch_vote(hough_ctx* c, uint32_t first_event, uint32_t n_events, uint16_t* d_count, uint16_t* d_mask,
+                        cudaStream_t st);
 cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,
                          uint32_t l_min, hough_peak* d_peaks, uint32_t* d_n_peaks, cudaStream_t st);
 cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
