@@ -214,7 +214,9 @@ def run_ours(args):
 
     w = make_workload(args.workload, args.events)
     E = w.n_events
-    chunk = min(args.chunk, E)
+    # events per vote/peaks/jets launch: --chunk, else as many as fit in about 34 GB of planes (C5: 128 events)
+    chunk = args.chunk if args.chunk > 0 else max(1, int(34.4e9 // (4 * w.bins_per_event)))
+    chunk = min(chunk, E)
     mode = "3d" if w.n_d0 > 1 else "2d"
     # weak scaling: every rank owns a batch of E events (event indices continue across ranks)
     batch = W.generate(w, E, first_event=rank * E)
@@ -380,7 +382,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (0 = the config's)")
-    ap.add_argument("--chunk", type=int, default=128, help="events per vote/peaks/jets launch")
+    ap.add_argument("--chunk", type=int, default=0, help="events per vote/peaks/jets launch (0: what fits in 34 GB of planes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

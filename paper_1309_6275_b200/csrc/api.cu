@@ -37,7 +37,7 @@ void free_all(hough_ctx* c)
 {
     cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
     cudaFree(c->d_rec); cudaFree(c->d_rec_u); cudaFree(c->d_key); cudaFree(c->d_seg); cudaFree(c->d_btab);
-    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status);
+    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
@@ -165,6 +165,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemcpy(c->d_d0sq, d0sq.data(), ND * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
     A(cudaMemset(c->d_status, 0, 8));
+    A(dev_alloc(&c->d_tilectr, 2));
+    A(cudaMemset(c->d_tilectr, 0, 8));
     for (int i = 0; i < 4; ++i) A(cudaEventCreate(&c->ev[i]));
     if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
     *out = c;

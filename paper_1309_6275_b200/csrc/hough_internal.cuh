@@ -57,6 +57,7 @@ struct hough_ctx {
     uint32_t* d_layer_r;                      // [2*16] float bits: min r, max r per layer
     TileWin* d_tilewin;                       // [16][n_strips]
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
+    uint32_t* d_tilectr;                      // [2]: vote kernel tile ticket + finished-block count (zero between launches)
     uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
     uint16_t* d_grpcnt;                       // [max_events][ceil(bins/256)] peaks per group of 256 / 512 bins
     uint64_t* d_jetkeys;                      // [max_events][max_peaks]

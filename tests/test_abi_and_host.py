@@ -68,6 +68,27 @@ def test_config_struct_layout_matches_header():
     assert vals[5] == B.JET_DTYPE.itemsize == 20
 
 
+def test_packed_sweep_keeps_every_rounding_of_o2():
+    """ptxas contracts mul.rn.f32x2 feeding add.rn.f32x2 into one FFMA2 (one rounding instead of the two O-2 asks
+    for).  The 3D sweep therefore forms a = two_d0 * rs with scalar FMULs; what must survive in the SASS of every
+    3D vote kernel is, per candidate pair, the three packed sums t, b, den (FADD2) next to the one round-down add
+    of the bin floor (FADD2.RM), and no packed multiply may have been fused away: NQ0 and u stay FMUL2."""
+    from paper_1309_6275_b200 import build
+    lib = build.build()
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
+    kernels = [b for b in sass.split("Function : ")[1:] if "vote_kernelILb1E" in b.split("\n")[0]]
+    assert len(kernels) == 3
+    for body in kernels:
+        n_rm = len(re.findall(r"\bFADD2\.RM\b", body))
+        n_add = len(re.findall(r"\bFADD2 ", body))
+        n_mul = len(re.findall(r"\bFMUL2 ", body))
+        n_fma = len(re.findall(r"\bFFMA2 ", body))
+        assert n_rm > 0
+        assert n_add == 3 * n_rm, (n_add, n_rm)
+        assert n_mul == 2 * n_rm, (n_mul, n_rm)
+        assert n_fma == 5 * n_rm, (n_fma, n_rm)
+
+
 def test_product_path_never_touches_the_oracle():
     """No file of the package (or bench's product arm) imports oracle/; the oracle never imports the package."""
     pkg = os.path.join(ROOT, "paper_1309_6275_b200")
