@@ -28,9 +28,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# FP32-pipe instructions per candidate of the normative O-2 sequence as compiled for sm_100a (DESIGN.md
-# "Roofline of the vote kernel"; counted from profiles/vote_kernel_sass_r01.txt): 3D = t, 2t, a, b, den,
-# 5 FFMA + FCHK of the IEEE division, v, u, 2 FSETP; 2D = m1, m2, s, 2s, division, v, u, 2 FSETP.
+# FP32-pipe instructions per vote of the normative O-2 sequence in scalar form: 3D = t, a, b,
+# den, the 6 FMA-pipe instructions of the IEEE division, v, u, the floor add + the per-hit m1, m2, s, rs, r2 shared by
+# the rows of a lane; 2D = m1, m2, s, division, v, u, floor.  (The kernel issues them two per instruction.)
 I_FP32 = {"3d": 15.0, "2d": 15.0}
 SM_COUNT, FP32_LANES = 148, 128
 
@@ -332,13 +332,16 @@ def run_ours(args):
     t_hbm = 4.0 * bins * E * args.steps / (hbm_gbs * 1e9)
     t_fp32 = votes_timed * I_FP32[mode] / fp32_peak
     bound = "alu" if t_fp32 >= t_hbm else "hbm"
+    # dram__bytes_read.sum + dram__bytes_write.sum of one vote launch (ncu --set full, profiles/r01b_summary.md);
+    # only known for the launch shape that capture was taken on (C5, 128 events per launch)
+    traffic = 34.33 if (w.name.startswith("C5") and chunk == 128) else None
     if bound == "alu":
         roofline = {"bound": "alu", "achieved": achieved_instr / 1e12, "peak": fp32_peak / 1e12, "unit": "Tinstr/s",
                     "frac": achieved_instr / fp32_peak, "traffic": None}
     else:
         ach = 4.0 * bins * E * args.steps / vote_s / 1e9
         roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
-                    "traffic": None}
+                    "traffic": traffic, "traffic_unit": "GB per launch (algorithmic: %.2f)" % (4.0 * bins * chunk / 1e9)}
     roofline.update({"kernel": "vote_kernel", "peak_source": peak_src + "; FP32 peak = 148 SM x 128 lanes x sm_max clock",
                      "ms_per_launch": ms_vote / max(1, len(stage_events)), "launches": len(stage_events),
                      "i_fp32_per_vote": I_FP32[mode], "t_bound_terms_ms": {"fp32": t_fp32 * 1e3, "hbm_write": t_hbm * 1e3},
