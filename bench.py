@@ -332,7 +332,7 @@ def run_ours(args):
     t_hbm = 4.0 * bins * E * args.steps / (hbm_gbs * 1e9)
     t_fp32 = votes_timed * I_FP32[mode] / fp32_peak
     bound = "alu" if t_fp32 >= t_hbm else "hbm"
-    # dram__bytes_read.sum + dram__bytes_write.sum of one vote launch (ncu --set full, profiles/r01b_summary.md);
+    # dram__bytes_read.sum + dram__bytes_write.sum of one vote launch (ncu --set full, profiles/r01c_summary.md);
     # only known for the launch shape that capture was taken on (C5, 128 events per launch)
     traffic = 34.33 if (w.name.startswith("C5") and chunk == 128) else None
     if bound == "alu":

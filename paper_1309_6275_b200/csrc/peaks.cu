@@ -12,8 +12,8 @@
 // resident SM keeps 2048 threads x kUnroll x 32 B = 256 KB in flight: the pass is bound by HBM, not by
 // instruction issue (about 12 warp instructions per KB).  Per unit the packed
 // 16-bit maximum (VIMNMX3.U16x2) is compared with l_min; only bins with count >= l_min (rare at the trigger
-// thresholds) run the 8 / 26-neighbour test, whose neighbour reads go to L2 (the neighbouring rows and d0
-// slabs were streamed by neighbouring warps a moment earlier), and only local maxima read the mask plane.
+// thresholds) read their mask word and, if popcount(mask) >= l_min, run the 8 / 26-neighbour test, whose reads
+// go to L2 (the neighbouring rows and d0 slabs were streamed by neighbouring warps a moment earlier).
 // Output: one bit per bin, written only for groups that hold a peak, and a peak count per group.
 // Compaction kernel: one block per event scans the group counts in linear-index order (block prefix sum,
 // 8 groups per thread) and writes the first max_peaks records; n_peaks is the true total.
