@@ -134,7 +134,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
     A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
     A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS));
-    A(dev_alloc(&c->d_tilewin, (size_t)HOUGH_MAX_LAYERS * c->vote.n_strips));
+    A(dev_alloc(&c->d_tilewin, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
     A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
