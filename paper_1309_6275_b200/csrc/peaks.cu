@@ -8,9 +8,9 @@
 // Stencil kernel = one streaming pass over the count plane.  The plane of an event is cut, in linear-index
 // order, into units of UB bins (UB = 16: one 256-bit load per lane; UB = 8: one 128-bit load when the plane is
 // not a whole number of 32-byte units) and groups of 32 units (one warp-wide load: 1 KB or 512 B, contiguous).
-// A warp takes kUnroll consecutive groups per iteration, all loads issued before the first use, so that a
-// resident SM keeps 2048 threads x kUnroll x 32 B = 256 KB in flight: the pass is bound by HBM, not by
-// instruction issue (about 12 warp instructions per KB).  Per unit the packed
+// A warp takes kUnroll consecutive groups per iteration and has the loads of its next iteration in flight while
+// it examines the current one (software pipeline): the pass is bound by HBM, not by instruction issue (about 3
+// thread instructions per bin).  Per unit the packed
 // 16-bit maximum (VIMNMX3.U16x2) is compared with l_min; only bins with count >= l_min (rare at the trigger
 // thresholds) read their mask word and, if popcount(mask) >= l_min, run the 8 / 26-neighbour test, whose reads
 // go to L2 (the neighbouring rows and d0 slabs were streamed by neighbouring warps a moment earlier).
@@ -42,7 +42,6 @@ struct PeakParams {
     uint32_t groups;             // per event = ceil(units / 32)
     uint32_t quads;              // per event = ceil(groups / kUnroll)
     uint32_t l_min;
-    uint32_t row_aligned;        // n_kappa % UB == 0: a unit never straddles two kappa rows
 };
 
 __device__ __forceinline__ void load_unit(const uint16_t* p, uint32_t (&r)[8])
@@ -113,20 +112,17 @@ __device__ __noinline__ bool is_peak(const uint16_t* __restrict__ cnt_e, const u
     return b0 && b1 && b2 && c0 && c1 && c2;
 }
 
-// Bins of one unit with count >= l_min that are not beaten by a neighbour INSIDE the unit (left must be strictly
-// smaller, right may tie).  Only valid when a unit never straddles two kappa rows (n_kappa % UB == 0).
+// Bit j set: bin j of the unit has count >= l_min (packed 16-bit compare, two bins per instruction).  On the
+// accumulators of the five configs a neighbour inside the unit almost never beats such a bin (1 % at C4), so no
+// in-register neighbour prefilter: the mask test that follows rejects far more (99.5 % at C4) for one load.
 template <int NW>
-__device__ __forceinline__ uint32_t unit_candidates(const uint32_t (&d)[NW], uint32_t l_min, bool row_aligned)
+__device__ __forceinline__ uint32_t unit_candidates(const uint32_t (&d)[NW], uint32_t lmin2)
 {
     uint32_t bits = 0;
-    uint32_t prev = 0;
 #pragma unroll
-    for (int j = 0; j < 2 * NW; ++j) {
-        const uint32_t c = (d[j >> 1] >> ((j & 1) * 16)) & 0xffffu;
-        const uint32_t next = (j + 1 < 2 * NW) ? ((d[(j + 1) >> 1] >> (((j + 1) & 1) * 16)) & 0xffffu) : 0u;
-        const bool inside = !row_aligned || (prev < c && next <= c);
-        if (c >= l_min && inside) bits |= 1u << j;
-        prev = c;
+    for (int w = 0; w < NW; ++w) {
+        const uint32_t t = __vcmpgeu2(d[w], lmin2) & 0x00010001u;   // bit 0: low bin, bit 16: high bin
+        bits |= ((t | (t >> 15)) & 3u) << (2 * w);
     }
     return bits;
 }
@@ -140,21 +136,34 @@ __global__ void __launch_bounds__(kStencilThreads, STENCIL_MINB) peak_stencil_ke
     const uint32_t gw = blockIdx.x * (kStencilThreads / 32) + (threadIdx.x >> 5);
     const uint64_t total_quads = (uint64_t)p.n_events * p.quads;
 
+    // software pipeline: the loads of the next iteration are in flight while this one is examined (on dense
+    // accumulators the candidates' mask loads would otherwise serialise with the stream)
+    auto load_quad = [&](uint64_t q, uint32_t (&dst)[kUnroll][NW]) {
+        const uint32_t e = (uint32_t)(q / p.quads);
+        const uint32_t g0 = (uint32_t)(q - (uint64_t)e * p.quads) * kUnroll;
+        const uint16_t* cnt_e = p.count + (size_t)e * p.bins;
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u) {
+            const uint32_t unit = (g0 + u) * 32u + lane;
+            if (unit < p.units) load_unit(cnt_e + (size_t)unit * UB, dst[u]);
+            else {
+#pragma unroll
+                for (int w = 0; w < NW; ++w) dst[u][w] = 0;
+            }
+        }
+    };
+    uint32_t d[kUnroll][NW], dn[kUnroll][NW];
+    if (gw < total_quads) load_quad(gw, dn);
     for (uint64_t q = gw; q < total_quads; q += n_warps) {
         const uint32_t e = (uint32_t)(q / p.quads);
         const uint32_t qi = (uint32_t)(q - (uint64_t)e * p.quads);
         const uint16_t* cnt_e = p.count + (size_t)e * p.bins;
         const uint32_t g0 = qi * kUnroll;
-        uint32_t d[kUnroll][NW];
 #pragma unroll
-        for (int u = 0; u < kUnroll; ++u) {
-            const uint32_t unit = (g0 + u) * 32u + lane;
-            if (unit < p.units) load_unit(cnt_e + (size_t)unit * UB, d[u]);
-            else {
+        for (int u = 0; u < kUnroll; ++u)
 #pragma unroll
-                for (int w = 0; w < NW; ++w) d[u][w] = 0;
-            }
-        }
+            for (int w = 0; w < NW; ++w) d[u][w] = dn[u][w];
+        if (q + n_warps < total_quads) load_quad(q + n_warps, dn);
         uint32_t m = packed_max(d[0]);
 #pragma unroll
         for (int u = 1; u < kUnroll; ++u) { const uint32_t t = packed_max(d[u]); m = __vimax3_u16x2(m, t, t); }
@@ -163,11 +172,12 @@ __global__ void __launch_bounds__(kStencilThreads, STENCIL_MINB) peak_stencil_ke
 #pragma unroll
         for (int u = 0; u < kUnroll; ++u) bits[u] = 0;
         if (ge) {                                                // some bin of this lane may be a peak
+            const uint32_t lmin2 = p.l_min | (p.l_min << 16);
             const uint16_t* msk_e = p.mask + (size_t)e * p.bins;
             uint32_t cand[kUnroll], mfirst[kUnroll];
 #pragma unroll
             for (int u = 0; u < kUnroll; ++u)
-                cand[u] = any_half_ge(packed_max(d[u]), p.l_min) ? unit_candidates<NW>(d[u], p.l_min, p.row_aligned != 0) : 0u;
+                cand[u] = unit_candidates<NW>(d[u], lmin2);
             // the mask words of the first candidate of every unit are fetched together (dense accumulators: most
             // units with a candidate have exactly one, and its mask rejects it), then the survivors are tested
 #pragma unroll
@@ -320,7 +330,6 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
     // 256-bit loads need 32-byte aligned units: every event plane starts at a multiple of 32 bytes iff the
     // caller's base pointer does and bins % 16 == 0
     const int ub = (pp.unit_bins == 16 && (((uintptr_t)d_count) & 31u) == 0) ? 16 : 8;
-    p.row_aligned = (c->cfg.n_kappa % (uint32_t)ub == 0) ? 1u : 0u;
     p.units = p.bins / (uint32_t)ub;
     p.groups = (p.units + 31u) / 32u;
     p.quads = (p.groups + kUnroll - 1) / kUnroll;
