@@ -245,6 +245,8 @@ __global__ void __launch_bounds__(kCompactThreads) peak_compact_kernel(const uin
     const uint16_t* msk_e = mask + (size_t)e * bins;
     hough_peak* out = peaks + (size_t)e * max_peaks;
     const uint32_t group_bytes = group_bins / 8;
+    // 32-bit reads of a group's bitmap: groups are at most 64 bytes, and word aligned if the event's bitmap is
+    const bool words_ok = group_bytes <= 64u && (group_bytes & 3u) == 0u && ((reinterpret_cast<uintptr_t>(bm) & 3u) == 0);
     uint32_t running = 0;
     for (uint32_t base = 0; base < groups; base += kCompactThreads * kGroupsPerThread) {
         const uint32_t g_first = base + (uint32_t)tid * kGroupsPerThread;
@@ -283,15 +285,34 @@ __global__ void __launch_bounds__(kCompactThreads) peak_compact_kernel(const uin
                 const uint8_t* gp = bm + (size_t)g * group_bytes;
                 const uint32_t lin_g = g * group_bins;
                 const uint32_t nbytes = min(group_bytes, bins / 8 - g * group_bytes);     // ragged last group
-                for (uint32_t b = 0; b < nbytes && pos < max_peaks; ++b) {
-                    uint32_t byte = gp[b];
-                    while (byte && pos < max_peaks) {
-                        const int qb = __ffs(byte) - 1;
-                        byte &= byte - 1;
-                        const uint32_t lin = lin_g + b * 8 + qb;
-                        hough_peak pk;
-                        pk.lin = lin; pk.count = cnt_e[lin]; pk.mask = msk_e[lin];
-                        out[pos++] = pk;
+                if (words_ok && (nbytes & 3u) == 0u) {                  // the group's bitmap as 32-bit words, all loads first
+                    const uint32_t* gw = reinterpret_cast<const uint32_t*>(gp);
+                    uint32_t wv[16];
+#pragma unroll
+                    for (int w = 0; w < 16; ++w) wv[w] = ((uint32_t)w * 4u < nbytes) ? __ldg(gw + w) : 0u;
+#pragma unroll
+                    for (int w = 0; w < 16; ++w) {
+                        uint32_t word = wv[w];
+                        while (word && pos < max_peaks) {
+                            const int qb = __ffs(word) - 1;
+                            word &= word - 1;
+                            const uint32_t lin = lin_g + (uint32_t)w * 32u + qb;
+                            hough_peak pk;
+                            pk.lin = lin; pk.count = cnt_e[lin]; pk.mask = msk_e[lin];
+                            out[pos++] = pk;
+                        }
+                    }
+                } else {
+                    for (uint32_t b = 0; b < nbytes && pos < max_peaks; ++b) {
+                        uint32_t byte = gp[b];
+                        while (byte && pos < max_peaks) {
+                            const int qb = __ffs(byte) - 1;
+                            byte &= byte - 1;
+                            const uint32_t lin = lin_g + b * 8 + qb;
+                            hough_peak pk;
+                            pk.lin = lin; pk.count = cnt_e[lin]; pk.mask = msk_e[lin];
+                            out[pos++] = pk;
+                        }
                     }
                 }
             }
