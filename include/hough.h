@@ -156,6 +156,9 @@ int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);
  *   kind 1: dependent-free fp32 non-FMA arithmetic (FADD/FMUL)                      -> thread-instructions / s
  *   kind 2: HBM read  (sum-reduce a buffer of `bytes`)                              -> bytes / s
  *   kind 3: HBM write (fill a buffer of `bytes`)                                    -> bytes / s
+ *   kind 4: packed fp32x2 non-FMA arithmetic (FMUL2/FADD2, register operands)       -> packed thread-instructions / s
+ *   kind 5: stores of all SMs into an L2-resident buffer, fully coalesced           -> bytes / s
+ *   kind 6: the same with the vote flush's pattern (64 B per lane pair, 1 KB rows)  -> bytes / s
  * `bytes` is only used by kinds 2 and 3.  HOST out.
  */
 int hough_microbench(int kind, size_t bytes, double* host_rate);

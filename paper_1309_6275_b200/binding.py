@@ -82,7 +82,8 @@ def _check(code: int, where: str):
 
 
 def microbench(kind: int, nbytes: int = 0) -> float:
-    """hough_microbench: 0 shared atomics/s, 1 fp32 non-FMA instr/s, 2 HBM read B/s, 3 HBM write B/s."""
+    """hough_microbench: 0 shared atomics/s, 1 fp32 non-FMA instr/s, 2 HBM read B/s, 3 HBM write B/s,
+    4 packed fp32x2 instr/s, 5 / 6 bytes/s all SMs can store into L2 (coalesced / vote-flush pattern)."""
     out = C.c_double(0.0)
     _check(load_library().hough_microbench(kind, nbytes, C.byref(out)), "hough_microbench")
     return out.value

@@ -32,7 +32,7 @@ __global__ void __launch_bounds__(1024) mb_fp32(int iters, float seed, float* si
 {
     float a0 = seed + threadIdx.x, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f;
     float a4 = a0 + 4.f, a5 = a0 + 5.f, a6 = a0 + 6.f, a7 = a0 + 7.f;
-    const float m = 0.999999f, c = 1e-3f;
+    const float m = 0.999999f + seed * 1e-9f, c = 1e-3f + seed * 1e-9f;     // register operands, as in the vote sweep
     for (int i = 0; i < iters; ++i) {
         a0 = __fmul_rn(a0, m); a1 = __fadd_rn(a1, c); a2 = __fmul_rn(a2, m); a3 = __fadd_rn(a3, c);
         a4 = __fmul_rn(a4, m); a5 = __fadd_rn(a5, c); a6 = __fmul_rn(a6, m); a7 = __fadd_rn(a7, c);
@@ -63,11 +63,59 @@ __global__ void __launch_bounds__(512) mb_write(uint4* __restrict__ dst, size_t 
         dst[i] = make_uint4((uint32_t)i, 1u, 2u, 3u);
 }
 
+// kind 4: packed fp32x2 non-FMA arithmetic (FMUL2 / FADD2 with register operands), 8 independent chains per thread
+__device__ __forceinline__ uint64_t mb_pk(float lo, float hi)
+{
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__global__ void __launch_bounds__(1024) mb_fp32x2(int iters, float seed, float* sink)
+{
+    uint64_t a[8];
+    for (int i = 0; i < 8; ++i) a[i] = mb_pk(seed + threadIdx.x + i, seed + threadIdx.x + i + 0.5f);
+    const uint64_t m = mb_pk(0.999999f + seed * 1e-9f, 0.999998f), c = mb_pk(1e-3f + seed * 1e-9f, 2e-3f);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; i += 2) {                         // a product never feeds a sum: ptxas would contract
+            asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(a[i]) : "l"(m));
+            asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a[i + 1]) : "l"(c));
+            asm volatile("mul.rn.f32x2 %0, %0, %1;" : "+l"(a[i]) : "l"(m));
+            asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a[i + 1]) : "l"(c));
+        }
+    }
+    uint64_t x = 0;
+    for (int i = 0; i < 8; ++i) x ^= a[i];
+    if (x == 0x12345ull) sink[0] = 1.f;
+}
+
+// kinds 5, 6: what one SM can store towards L2 (the buffer is small enough to stay in L2: no DRAM limit).  Every
+// block rewrites its own 128 KB; kind 5 fully coalesced 128-bit stores, kind 6 the pattern of the vote flush (256-bit
+// stores, lane pairs write 64 contiguous bytes of rows 1 KB apart).
+template <bool FLUSH_PATTERN>
+__global__ void __launch_bounds__(1024) mb_store(unsigned char* buf, int iters)
+{
+    unsigned char* base = buf + (size_t)blockIdx.x * 131072;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int it = 0; it < iters; ++it) {
+        if (!FLUSH_PATTERN) {
+            for (int o = threadIdx.x * 16; o < 131072; o += 1024 * 16) *reinterpret_cast<uint4*>(base + o) = make_uint4(it, 1, 2, 3);
+        } else {
+            for (int g = 0; g < 4; ++g)
+                for (int kb = warp; kb < 16; kb += 32) {
+                    unsigned char* q = base + g * 32768 + (lane & ~1) * 1024 + kb * 64 + (lane & 1) * 32;
+                    asm volatile("st.global.cs.v8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" :: "l"(q), "r"(it) : "memory");
+                    asm volatile("st.global.cs.v8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" :: "l"(q + 1024), "r"(it) : "memory");
+                }
+        }
+    }
+}
+
 }  // namespace
 
 extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
 {
-    if (!host_rate || kind < 0 || kind > 3) return HOUGH_EINVAL;
+    if (!host_rate || kind < 0 || kind > 6) return HOUGH_EINVAL;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ECUDA;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -79,7 +127,8 @@ extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
     double work = 0.0;
     float best_ms = 1e30f;
     const int reps = 5;
-    if (kind >= 2) {
+    if (kind == 5 || kind == 6) bytes = (size_t)sms * 131072;
+    if (kind == 2 || kind == 3 || kind == 5 || kind == 6) {
         if (bytes < (1u << 20)) bytes = (size_t)1 << 30;
         if (cudaMalloc(&buf, bytes) != cudaSuccess) { cudaFree(sink); return HOUGH_ENOMEM; }
         cudaMemset(buf, 1, bytes);
@@ -94,6 +143,15 @@ extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
             const int iters = 8192;
             mb_fp32<<<sms * 2, 1024>>>(iters, 1.0f, (float*)sink);
             work = (double)sms * 2 * 1024 * iters * 16;
+        } else if (kind == 4) {
+            const int iters = 8192;
+            mb_fp32x2<<<sms * 2, 1024>>>(iters, 1.0f, (float*)sink);
+            work = (double)sms * 2 * 1024 * iters * 16;          // packed instructions (two operations each)
+        } else if (kind == 5 || kind == 6) {
+            const int iters = 2000;
+            if (kind == 5) mb_store<false><<<sms, 1024>>>((unsigned char*)buf, iters);
+            else mb_store<true><<<sms, 1024>>>((unsigned char*)buf, iters);
+            work = (double)sms * 131072.0 * iters;               // bytes, all SMs together
         } else if (kind == 2) {
             mb_read<<<sms * 8, 512>>>((const uint4*)buf, bytes / 16, sink);
             work = (double)bytes;
