@@ -71,8 +71,9 @@ enum {
 /*
  * Create a context.  HOST pointers.  Validates cfg, builds the constant tables in double precision
  * (cos/sin of the phi0 bin centres, d0 bin centres, 2*d0, d0^2, NK/(2*kappa_max)), rounds each once to
- * fp32, uploads them, and allocates the workspaces (prepared hits: 20 B per hit; peak bitmap: 1 bit per
- * bin per event; jet keys: 8 B per stored peak; optional host-path planes).  Synchronous.
+ * fp32, uploads them, and allocates the workspaces (prepared hits: 36 B per hit = sorted record 16 B +
+ * unsorted record 16 B + sort key 4 B, plus 9 B per hit of staging if host_chunk_events > 0; peak bitmap:
+ * 1 bit per bin per event; jet keys: 8 B per stored peak; optional host-path planes).  Synchronous.
  */
 int hough_create(const hough_config* cfg, hough_ctx** out);
 int hough_destroy(hough_ctx* ctx);
@@ -162,6 +163,23 @@ int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);
  * `bytes` is only used by kinds 2 and 3.  HOST out.
  */
 int hough_microbench(int kind, size_t bytes, double* host_rate);
+
+/*
+ * Debug exports (synchronous, HOST out; not part of the hot path).
+ *
+ * hough_debug_prepared_hits: the prepared records of the LAST hough_vote / hough_trigger_host call on ctx, in the
+ *   caller's hit order: h_rec[4*h + 0..3] = {RN32(sin phi_h), RN32(cos phi_h), r_h, bit pattern 0x10000 << layer_h}
+ *   (O-1; hits that are ignored -- layer >= n_layers or non-finite phi -- read {0, 1, r, 0}).  Lets a test compare
+ *   sp / cp bit for bit with the oracle's (reading R6: the residual double-rounding risk that
+ *   HOUGH_ST_TRIG_ROUNDING reports).  h_trig_risk (may be null) receives the number of hits the device flagged.
+ * hough_debug_div_check: runs the vote kernel's branch-free division and packed O-2 tail next to the plain IEEE
+ *   reference (__fdiv_rn, scalar tail) on n_pairs generated operand pairs (tame range, rounding midpoints, bin
+ *   edges, vanishing denominators) for a kappa axis of n_kappa bins over +-kappa_max.
+ *   h_out[0] = quotients that differ in any bit, h_out[1] = bin decisions that differ, h_out[2] = pairs that
+ *   landed inside the axis (the test is not vacuous).  DESIGN.md readings R31-R33.
+ */
+int hough_debug_prepared_hits(hough_ctx* ctx, uint64_t n_hits, float* h_rec /* [n_hits][4] */, uint32_t* h_trig_risk);
+int hough_debug_div_check(uint64_t n_pairs, uint64_t seed, float kappa_max, uint32_t n_kappa, uint64_t* h_out /* [3] */);
 
 const char* hough_strerror(int code);
 

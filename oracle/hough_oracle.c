@@ -78,6 +78,18 @@ void oracle_tables(const oracle_grid *g, float *c0, float *s0, float *d0c, float
     *inv_dk = inv_dkappa(g);
 }
 
+/* ---- O-1 hit preparation: sin/cos of the hit azimuth, evaluated in double and rounded once to fp32 ---- */
+/* (reading R6: the correctly-rounded fp32 of the real value, obtained by fp64 evaluation + one rounding) */
+
+static float hit_sin(float phi) { return (float)sin((double)phi); }
+static float hit_cos(float phi) { return (float)cos((double)phi); }
+
+/* exported so a test can compare the CUDA path's prepared records with these values bit for bit (R6) */
+void oracle_hit_prep(uint64_t n_hits, const float *phi, float *sp, float *cp)
+{
+    for (uint64_t h = 0; h < n_hits; ++h) { sp[h] = hit_sin(phi[h]); cp[h] = hit_cos(phi[h]); }
+}
+
 /* ---- O-2: one candidate (hit, id, ip) -> kappa bin, or -1 if it does not vote ------------------ */
 /* Every statement below is exactly one IEEE fp32 operation (compiled with -ffp-contract=off).      */
 
@@ -129,8 +141,8 @@ int64_t oracle_vote(const oracle_grid *g, uint64_t n_hits, const float *r, const
     oracle_tables(g, c0, s0, d0c, &inv_dk_unused);
     for (uint64_t h = 0; h < n_hits; ++h) {
         if (layer[h] >= g->n_layers) continue;                 /* R9: invalid hit ignored */
-        const float sp = (float)sin((double)phi[h]);           /* O-1 */
-        const float cp = (float)cos((double)phi[h]);
+        const float sp = hit_sin(phi[h]);                      /* O-1 */
+        const float cp = hit_cos(phi[h]);
         const float rr = r[h];
         const float r2 = rr * rr;
         const uint16_t bit = (uint16_t)(1u << layer[h]);
@@ -165,8 +177,8 @@ int64_t oracle_vote_columns(const oracle_grid *g, uint64_t n_hits, const float *
     int64_t votes = 0;
     for (uint64_t h = 0; h < n_hits; ++h) {
         if (layer[h] >= g->n_layers) continue;
-        const float sp = (float)sin((double)phi[h]);
-        const float cp = (float)cos((double)phi[h]);
+        const float sp = hit_sin(phi[h]);
+        const float cp = hit_cos(phi[h]);
         const float rr = r[h];
         const float r2 = rr * rr;
         const uint16_t bit = (uint16_t)(1u << layer[h]);

@@ -51,6 +51,8 @@ def _load():
         p = C.c_void_p
         lib.oracle_tables.argtypes = [C.POINTER(_Grid), p, p, p, p]
         lib.oracle_tables.restype = None
+        lib.oracle_hit_prep.argtypes = [C.c_uint64, p, p, p]
+        lib.oracle_hit_prep.restype = None
         lib.oracle_vote.argtypes = [C.POINTER(_Grid), C.c_uint64, p, p, p, C.c_uint32, C.c_uint32,
                                     C.c_uint32, C.c_uint32, p, p]
         lib.oracle_vote.restype = C.c_int64
@@ -110,6 +112,14 @@ def _hits(r, phi, layer):
     layer = np.ascontiguousarray(layer, np.uint8)
     assert r.shape == phi.shape == layer.shape and r.ndim == 1
     return r, phi, layer
+
+
+def hit_prep(phi):
+    """O-1 for an array of hit azimuths: (sp, cp) = fp32 roundings of sin / cos evaluated in double (reading R6)."""
+    phi = np.ascontiguousarray(phi, np.float32)
+    sp = np.zeros(phi.size, np.float32); cp = np.zeros(phi.size, np.float32)
+    _load().oracle_hit_prep(phi.size, _ptr(phi), _ptr(sp), _ptr(cp))
+    return sp, cp
 
 
 def vote(g: Grid, r, phi, layer, id_range: Optional[Tuple[int, int]] = None,

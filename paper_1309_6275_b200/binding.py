@@ -22,7 +22,8 @@ JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced"
 
 ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING = 1, 2, 4
 EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_jets",
-           "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror"]
+           "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
+           "hough_debug_prepared_hits", "hough_debug_div_check"]
 
 
 class HoughConfig(C.Structure):
@@ -63,6 +64,8 @@ def load_library() -> C.CDLL:
         lib.hough_status.argtypes = [p, C.POINTER(u32)]
         lib.hough_launch_count.argtypes = [p, C.POINTER(u64)]
         lib.hough_microbench.argtypes = [C.c_int, C.c_size_t, C.POINTER(C.c_double)]
+        lib.hough_debug_prepared_hits.argtypes = [p, u64, p, C.POINTER(u32)]
+        lib.hough_debug_div_check.argtypes = [u64, u64, f32, u32, C.POINTER(u64)]
         lib.hough_strerror.argtypes = [C.c_int]
         lib.hough_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -87,6 +90,13 @@ def microbench(kind: int, nbytes: int = 0) -> float:
     out = C.c_double(0.0)
     _check(load_library().hough_microbench(kind, nbytes, C.byref(out)), "hough_microbench")
     return out.value
+
+
+def debug_div_check(n_pairs: int, seed: int = 1, kappa_max: float = 0.3e-3 * 3.8, n_kappa: int = 512):
+    """hough_debug_div_check -> (quotient mismatches, bin mismatches, pairs inside the kappa axis)."""
+    out = (C.c_uint64 * 3)()
+    _check(load_library().hough_debug_div_check(n_pairs, seed, kappa_max, n_kappa, out), "hough_debug_div_check")
+    return int(out[0]), int(out[1]), int(out[2])
 
 
 def _dptr(t) -> C.c_void_p:
@@ -116,7 +126,10 @@ class Hough:
     def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
                      host_chunk_events: int = 0, max_peaks: Optional[int] = None) -> "Hough":
         ne = w.n_events if max_events is None else max_events
-        mh = max_hits if max_hits is not None else ne * 65535
+        if max_hits is None:
+            raise ValueError("for_workload: pass max_hits (the hit count of the largest batch per call); the context "
+                             "allocates 36 B of workspace per hit")
+        mh = max_hits
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
                    min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
                    host_chunk_events)
@@ -192,6 +205,14 @@ class Hough:
         out = C.c_uint32(0)
         _check(self.lib.hough_status(self._ctx, C.byref(out)), "hough_status")
         return out.value
+
+    def hough_debug_prepared_hits(self, n_hits: int):
+        """(records float32 [n_hits, 4] = sp, cp, r, layer-bit pattern; number of hits flagged trig-rounding risk)."""
+        rec = np.zeros((max(n_hits, 1), 4), np.float32)
+        risk = C.c_uint32(0)
+        _check(self.lib.hough_debug_prepared_hits(self._ctx, n_hits, C.c_void_p(rec.ctypes.data), C.byref(risk)),
+               "hough_debug_prepared_hits")
+        return rec[:n_hits], risk.value
 
     def hough_launch_count(self) -> int:
         out = C.c_uint64(0)

@@ -42,7 +42,8 @@ void free_all(hough_ctx* c)
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
     cudaFree(c->d_hp_jets); cudaFree(c->d_hp_npeaks); cudaFree(c->d_hp_njets); cudaFree(c->d_hp_flag);
-    for (int i = 0; i < 4; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (cudaEvent_t ev : c->ev_pool) cudaEventDestroy(ev);
+    c->ev_pool.clear();
 }
 
 bool config_ok(const hough_config* g)
@@ -91,9 +92,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         snprintf(g_errbuf, sizeof(g_errbuf), "device sm_%d%d is not sm_100-class", prop.major, prop.minor);
         return HOUGH_ECUDA;
     }
-    hough_ctx* c = new (std::nothrow) hough_ctx();
+    hough_ctx* c = new (std::nothrow) hough_ctx();          // value-initialised: every pointer null, every counter 0
     if (!c) return HOUGH_ENOMEM;
-    memset(c, 0, sizeof(*c));
     c->cfg = *cfg;
     c->device = dev;
     c->sm_count = prop.multiProcessorCount;
@@ -136,6 +136,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS));
     A(dev_alloc(&c->d_tilewin, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips));
     A(dev_alloc(&c->d_status, 2));
+    A(dev_alloc(&c->d_tilectr, 2));
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
     A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
     A(dev_alloc(&c->d_jetkeys, (size_t)cfg->max_events * cfg->max_peaks_per_event));
@@ -165,9 +166,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemcpy(c->d_d0sq, d0sq.data(), ND * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
     A(cudaMemset(c->d_status, 0, 8));
-    A(dev_alloc(&c->d_tilectr, 2));
     A(cudaMemset(c->d_tilectr, 0, 8));
-    for (int i = 0; i < 4; ++i) A(cudaEventCreate(&c->ev[i]));
     if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
     *out = c;
     return HOUGH_OK;
@@ -262,11 +261,18 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
     // hits are prepared once for the whole batch; the chunks then share the prepared records
     CK(launch_prep(ctx, n_events, ctx->d_hp_off, n_hits_total, ctx->d_hp_r, ctx->d_hp_phi, ctx->d_hp_layer, st), "hit preparation");
     const int cone_bins = cone_bins_of(cone_rad, g.n_phi0);
-    std::vector<cudaEvent_t> evs;
-    for (uint32_t e0 = 0; e0 < n_events; e0 += g.host_chunk_events) {
+    // stage timing uses events owned by the context (created once, reused by later calls, freed in hough_destroy)
+    const size_t n_chunks = ((size_t)n_events + g.host_chunk_events - 1) / g.host_chunk_events;
+    if (ms_stage)
+        while (ctx->ev_pool.size() < 4 * n_chunks) {
+            cudaEvent_t ev = nullptr;
+            CK(cudaEventCreate(&ev), "cudaEventCreate");
+            ctx->ev_pool.push_back(ev);
+        }
+    size_t chunk_i = 0;
+    for (uint32_t e0 = 0; e0 < n_events; e0 += g.host_chunk_events, ++chunk_i) {
         const uint32_t ne = (n_events - e0 < g.host_chunk_events) ? n_events - e0 : g.host_chunk_events;
-        cudaEvent_t t[4] = {nullptr, nullptr, nullptr, nullptr};
-        if (ms_stage) for (int i = 0; i < 4; ++i) { CK(cudaEventCreate(&t[i]), "event"); evs.push_back(t[i]); }
+        cudaEvent_t* t = ms_stage ? &ctx->ev_pool[4 * chunk_i] : nullptr;
         if (ms_stage) cudaEventRecord(t[0], st);
         CK(launch_vote(ctx, e0, ne, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel");
         if (ms_stage) cudaEventRecord(t[1], st);
@@ -290,14 +296,13 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
                            cudaMemcpyDeviceToHost, st), "D2H jets");
     CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
     if (ms_stage) {
-        for (size_t i = 0; i + 3 < evs.size(); i += 4)
+        for (size_t i = 0; i < 4 * n_chunks; i += 4)
             for (int s = 0; s < 3; ++s) {
                 float ms = 0.f;
-                cudaEventElapsedTime(&ms, evs[i + s], evs[i + s + 1]);
+                cudaEventElapsedTime(&ms, ctx->ev_pool[i + s], ctx->ev_pool[i + s + 1]);
                 ms_stage[s] += ms;
             }
     }
-    for (cudaEvent_t ev : evs) cudaEventDestroy(ev);
     return HOUGH_OK;
 }
 
@@ -309,6 +314,28 @@ int hough_status(hough_ctx* ctx, uint32_t* host_status_bits)
     CK(cudaMemcpy(st, ctx->d_status, 8, cudaMemcpyDeviceToHost), "hough_status copy");
     ctx->status_host |= st[0];
     *host_status_bits = ctx->status_host;
+    return HOUGH_OK;
+}
+
+int hough_debug_prepared_hits(hough_ctx* ctx, uint64_t n_hits, float* h_rec, uint32_t* h_trig_risk)
+{
+    if (!ctx || (n_hits > 0 && !h_rec) || n_hits > ctx->cfg.max_hits) return HOUGH_EINVAL;
+    CK(cudaStreamSynchronize(ctx->last_stream), "hough_debug_prepared_hits synchronize");
+    if (n_hits) CK(cudaMemcpy(h_rec, ctx->d_rec_u, n_hits * sizeof(float4), cudaMemcpyDeviceToHost), "prepared-hit copy");
+    if (h_trig_risk) {
+        uint32_t st[2] = {0, 0};
+        CK(cudaMemcpy(st, ctx->d_status, 8, cudaMemcpyDeviceToHost), "status copy");
+        *h_trig_risk = st[1];
+    }
+    return HOUGH_OK;
+}
+
+int hough_debug_div_check(uint64_t n_pairs, uint64_t seed, float kappa_max, uint32_t n_kappa, uint64_t* h_out)
+{
+    if (!h_out || !(kappa_max > 0.f) || n_kappa < 8 || n_kappa > (1u << 20)) return HOUGH_EINVAL;
+    unsigned long long out[3] = {0, 0, 0};
+    CK(run_div_check(n_pairs, seed, kappa_max, (int)n_kappa, out), "division check kernel");
+    for (int i = 0; i < 3; ++i) h_out[i] = out[i];
     return HOUGH_OK;
 }
 

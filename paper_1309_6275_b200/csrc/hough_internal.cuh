@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "hough.h"
 
 #define HOUGH_MAX_LAYERS 16
@@ -66,7 +68,7 @@ struct hough_ctx {
     uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
     hough_peak* d_hp_peaks; hough_track* d_hp_tracks; hough_jet* d_hp_jets;
     uint32_t* d_hp_npeaks; uint32_t* d_hp_njets; uint8_t* d_hp_flag;
-    cudaEvent_t ev[4];
+    std::vector<cudaEvent_t> ev_pool;         // hough_trigger_host stage timing: 4 per chunk, created on first use
     VotePlan vote;
     PeakPlan peak;
     cudaStream_t last_stream;
@@ -86,3 +88,4 @@ cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_pea
                         uint32_t* d_n_jets, uint8_t* d_flag, cudaStream_t st);
 cudaError_t plan_vote(hough_ctx* c);
 cudaError_t plan_peaks(hough_ctx* c);
+cudaError_t run_div_check(uint64_t n_pairs, uint64_t seed, float kmax, int nk, unsigned long long* host_out3);

@@ -119,10 +119,15 @@ extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return HOUGH_ECUDA;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaEvent_t t0, t1;
-    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    cudaEvent_t t0 = nullptr, t1 = nullptr;
     uint32_t* sink = nullptr;
-    cudaMalloc((void**)&sink, 16);
+    if (cudaEventCreate(&t0) != cudaSuccess || cudaEventCreate(&t1) != cudaSuccess ||
+        cudaMalloc((void**)&sink, 16) != cudaSuccess) {
+        if (t0) cudaEventDestroy(t0);
+        if (t1) cudaEventDestroy(t1);
+        cudaFree(sink);
+        return HOUGH_ECUDA;
+    }
     void* buf = nullptr;
     double work = 0.0;
     float best_ms = 1e30f;
@@ -130,7 +135,11 @@ extern "C" int hough_microbench(int kind, size_t bytes, double* host_rate)
     if (kind == 5 || kind == 6) bytes = (size_t)sms * 131072;
     if (kind == 2 || kind == 3 || kind == 5 || kind == 6) {
         if (bytes < (1u << 20)) bytes = (size_t)1 << 30;
-        if (cudaMalloc(&buf, bytes) != cudaSuccess) { cudaFree(sink); return HOUGH_ENOMEM; }
+        if (cudaMalloc(&buf, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(sink); cudaEventDestroy(t0); cudaEventDestroy(t1);
+            return HOUGH_ENOMEM;
+        }
         cudaMemset(buf, 1, bytes);
     }
     for (int rep = 0; rep < reps + 1; ++rep) {

@@ -575,3 +575,75 @@ def test_P12_hand_built_event_end_to_end(k_disp):
         a = np.abs(2 * (res.peaks["lin"][mem].astype(np.int64) % 128) - 127)
         assert res.jets["seed_track"][J] == mem[np.argmin(a)]
         assert abs(res.jets["sum_pt"][J] - res.tracks["pt"][mem].sum()) < 1e-4 * res.jets["sum_pt"][J]
+
+
+# ----------------------------------------------------------------------------------------------
+# P13: O-1 hit preparation = correctly rounded fp32 of the real sin / cos (reading R6)
+# ----------------------------------------------------------------------------------------------
+
+def _sincos_exact(x_f32, prec=70):
+    """sin and cos of the float32 value x to `prec` significant digits (Taylor series in decimal arithmetic)."""
+    import decimal
+    ctx = decimal.Context(prec=prec)
+    D = decimal.Decimal
+    # pi by Machin's formula, 16 atan(1/5) - 4 atan(1/239), in the same context
+    def atan_inv(n):
+        x = ctx.divide(D(1), D(n)); x2 = ctx.multiply(x, x)
+        term, total, k = x, x, 1
+        while True:
+            term = ctx.multiply(term, x2); k += 2
+            t = ctx.divide(term, D(k))
+            total = ctx.subtract(total, t) if (k // 2) % 2 else ctx.add(total, t)
+            if t.copy_abs() < D(10) ** (-prec - 5):
+                return total
+    pi = ctx.subtract(ctx.multiply(D(16), atan_inv(5)), ctx.multiply(D(4), atan_inv(239)))
+    x = D(float(x_f32))                                   # exact: every float is a finite decimal
+    two_pi = ctx.multiply(D(2), pi)
+    k = (x / two_pi).to_integral_value(rounding=decimal.ROUND_HALF_EVEN)
+    y = ctx.subtract(x, ctx.multiply(k, two_pi))          # |y| <= pi
+    y2 = ctx.multiply(y, y)
+    s, c, ts, tc, n = y, D(1), y, D(1), 1
+    while True:
+        tc = ctx.divide(ctx.multiply(tc, y2), D((2 * n - 1) * (2 * n)))
+        ts = ctx.divide(ctx.multiply(ts, y2), D((2 * n) * (2 * n + 1)))
+        if n % 2:
+            c = ctx.subtract(c, tc); s = ctx.subtract(s, ts)
+        else:
+            c = ctx.add(c, tc); s = ctx.add(s, ts)
+        n += 1
+        if max(tc.copy_abs(), ts.copy_abs()) < D(10) ** (-prec + 5):
+            return s, c
+
+
+def _round_to_f32(dec):
+    """Nearest float32 of an exact decimal value (ties cannot occur for transcendental values)."""
+    from fractions import Fraction
+    x = Fraction(dec)
+    f = np.float32(float(dec))
+    cands = [f, np.nextafter(f, np.float32(np.inf)), np.nextafter(f, np.float32(-np.inf))]
+    return min(cands, key=lambda c: abs(Fraction(float(c)) - x))
+
+
+def test_hit_prep_is_the_correctly_rounded_sine_and_cosine():
+    """O-1 / R6: (float)sin((double)phi) is the correctly rounded fp32 of the real sine (glibc's double sin is
+    accurate to < 1 ulp64, so the single rounding to fp32 is correct except within ~2^-29 of a tie).  Checked
+    against a 70-digit decimal Taylor series on azimuths in [0, 2pi), near multiples of pi/2, and outside the
+    principal range."""
+    rng = np.random.default_rng(13)
+    phi = np.concatenate([rng.uniform(0, TWO_PI, 300), np.arange(9) * (math.pi / 2), np.arange(9) * (math.pi / 2) + 1e-4,
+                          [1e-6, 3e-5, 6.2831, 6.283185, -7.5, 100.0, 0.0]]).astype(np.float32)
+    sp, cp = O.hit_prep(phi)
+    for x, a, b in zip(phi, sp, cp):
+        s, c = _sincos_exact(x)
+        assert a == _round_to_f32(s), (float(x), float(a))
+        assert b == _round_to_f32(c), (float(x), float(b))
+    # and it is what the vote itself uses, in the order sin(phi)cos(phi0c) - cos(phi)sin(phi0c): a hit at azimuth
+    # 1 rad gives s < 0 (kappa below the axis centre) in the column centred above it and s > 0 in the one below
+    g = O.Grid(64, 32)
+    cnt, _, _ = O.vote(g, np.float32([250.0]), np.float32([1.0]), np.uint8([0]))
+    ip = int(1.0 / (TWO_PI / 64))                          # column 10, centre 1.0308 rad > phi
+    k_up, k_dn = int(np.argmax(cnt[0, ip])), int(np.argmax(cnt[0, ip - 1]))
+    assert cnt[0, ip].sum() == 1 and cnt[0, ip - 1].sum() == 1 and k_up < 16 <= k_dn
+    for col, k in ((ip, k_up), (ip - 1, k_dn)):
+        u = (2.0 * math.sin(1.0 - (col + 0.5) * TWO_PI / 64) / 250.0 + KMAX) * 32 / (2 * KMAX)
+        assert int(u) == k
