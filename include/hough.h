@@ -43,8 +43,12 @@ typedef struct {
     uint64_t max_hits;             /* per call, total over events (sizes the prepared-hit workspace), < 2^32          */
     uint32_t max_peaks_per_event;  /* capacity of the per-event peak / track lists                                    */
     uint32_t max_jets_per_event;   /* capacity of the per-event jet list                                              */
-    uint32_t host_chunk_events;    /* hough_trigger_host only: events per internal chunk (the context then owns
-                                      2 * host_chunk_events * ND*NPHI*NK*2 bytes of accumulator planes); 0 disables   */
+    uint32_t host_chunk_events;    /* hough_trigger_host: events per internal launch; 0 disables that entry point.
+                                      If > 0 the context owns host staging buffers for max_events / max_hits, the
+                                      planes of ONE event (fallback for events that overflow the candidate buffer),
+                                      and hough_vote_peaks accepts at most host_chunk_events events per call        */
+    uint32_t max_candidates_per_event; /* fused path: capacity of the per-event peak-candidate buffer (16 B each);
+                                      0 = default max(4 * max_peaks_per_event, 4096)                                  */
 } hough_config;
 
 typedef struct { uint32_t lin; uint16_t count; uint16_t mask; } hough_peak;                     /*  8 B */
@@ -63,6 +67,8 @@ enum {
 enum {
     HOUGH_ST_EVENT_TOO_LARGE = 1u,   /* an event has > 65535 hits: its counts may wrap (uint16), results undefined  */
     HOUGH_ST_BAD_OFFSETS = 2u,       /* hit_offsets not non-decreasing or beyond n_hits_total                        */
+    HOUGH_ST_CANDIDATE_OVERFLOW = 8u,/* hough_vote_peaks: an event had more peak candidates than
+                                        max_candidates_per_event; its n_peaks reads HOUGH_N_PEAKS_OVERFLOW           */
     HOUGH_ST_TRIG_ROUNDING = 4u      /* informational: some sin/cos(phi) lay within a few fp64 ulps of an fp32
                                         rounding boundary, so its correctly-rounded fp32 value is not certain
                                         (reading R6; probability ~1e-8 per hit)                            */
@@ -115,6 +121,27 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
                 uint32_t l_min, hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream);
 
 /*
+ * A0-A4 fused  Vote -> peaks without the accumulator in HBM ("the hit data ... is
+ * processed using the Hough transform to compute the parameter space representation.  Candidate tracks are
+ * identified by finding local maxima", and PAPER.md:109: the transform is limited "more by memory access
+ * operations rather than the computational rate").  Same result as hough_vote followed by hough_peaks -- the same
+ * peaks, in ascending lin, with the same count / mask, and the true total -- but the vote kernel finds the peak
+ * candidates (popcount(mask) >= l_min) while its tile is in shared memory, compares them with the neighbours
+ * inside the tile, and a second kernel recomputes, from the hits, the few neighbour bins that lie across a tile
+ * border (O-2 verbatim, so the counts are the accumulator's).  No plane is written.
+ *   arguments as hough_vote / hough_peaks.  Capacity: if an event has more than max_candidates_per_event
+ *   candidates, HOUGH_ST_CANDIDATE_OVERFLOW is raised and d_n_peaks[e] = HOUGH_N_PEAKS_OVERFLOW (no record of
+ *   that event is valid; hough_jets treats it as an event without tracks): re-run such events through
+ *   hough_vote + hough_peaks (hough_trigger_host does).
+ * Returns HOUGH_EINVAL as hough_vote / hough_peaks do, and if n_events exceeds the fused capacity
+ * (host_chunk_events if that is > 0, else max_events).
+ */
+#define HOUGH_N_PEAKS_OVERFLOW 0xFFFFFFFFu
+int hough_vote_peaks(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets, uint64_t n_hits_total,
+                     const float* d_r, const float* d_phi, const uint8_t* d_layer, uint32_t l_min,
+                     hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream);
+
+/*
  * A5-A6  Peak -> track conversion and phi-cone track-jets ("measure ... the transverse momentum";
  * PAPER.md:113-123 jets / displaced jets, in north_star's phi-cone form).  For the T = min(n_peaks, max_peaks)
  * stored peaks of each event: track j = {pT = 0.3e-3*B/|kappa_c|, phi0_c, d0_c, q = -sign(kappa_c), jet};
@@ -132,10 +159,13 @@ int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, con
 
 /*
  * End-to-end trigger on HOST buffers (the call bench.py's e2e leg times): copies the hits to the device,
- * runs vote -> peaks -> jets in chunks of cfg.host_chunk_events events on the context's own planes, and
- * copies n_peaks / n_jets / flag (and, if non-null, peaks and jets) back.  All h_* pointers are HOST memory
- * (pinned memory makes the copies asynchronous); synchronises `stream` before returning.
- * ms_stage (HOST, may be null) receives the device time in ms spent in {vote, peaks, jets}.
+ * runs the fused vote -> peaks path and the jets in launches of cfg.host_chunk_events events, and copies
+ * n_peaks / n_jets / flag (and, if non-null, peaks and jets) back.  Events that overflowed the candidate buffer
+ * are re-run one by one through the accumulator path (hough_vote + hough_peaks on the context's one-event planes),
+ * so the results are always those of the definition.  All h_* pointers are HOST memory (pinned memory makes the
+ * copies asynchronous); synchronises `stream` before returning.
+ * ms_stage (HOST, may be null) receives the device time in ms spent in {vote (incl. candidate scan), peaks
+ * (recount + ordering), jets}.
  */
 int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
                        const float* h_r, const float* h_phi, const uint8_t* h_layer,

@@ -20,8 +20,11 @@ TRACK_DTYPE = np.dtype([("pt", "<f4"), ("phi0", "<f4"), ("d0", "<f4"), ("q", "<i
 JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced", "<u4"),
                       ("phi", "<f4"), ("sum_pt", "<f4")])
 
-ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING = 1, 2, 4
-EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_jets",
+ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING, ST_CANDIDATE_OVERFLOW = 1, 2, 4, 8
+ST_ERRORS = ST_EVENT_TOO_LARGE | ST_BAD_OFFSETS            # the bits that mean "results undefined"
+N_PEAKS_OVERFLOW = 0xFFFFFFFF
+EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_vote_peaks",
+           "hough_jets",
            "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
            "hough_debug_prepared_hits", "hough_debug_div_check"]
 
@@ -31,7 +34,7 @@ class HoughConfig(C.Structure):
                 ("kappa_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float), ("b_tesla", C.c_float),
                 ("n_layers", C.c_uint32), ("max_events", C.c_uint32), ("max_hits", C.c_uint64),
                 ("max_peaks_per_event", C.c_uint32), ("max_jets_per_event", C.c_uint32),
-                ("host_chunk_events", C.c_uint32)]
+                ("host_chunk_events", C.c_uint32), ("max_candidates_per_event", C.c_uint32)]
 
 
 class HoughError(RuntimeError):
@@ -59,6 +62,7 @@ def load_library() -> C.CDLL:
         lib.hough_plane_bytes.restype = C.c_size_t
         lib.hough_vote.argtypes = [p, u32, p, u64, p, p, p, p, p, p]
         lib.hough_peaks.argtypes = [p, u32, p, p, u32, p, p, p]
+        lib.hough_vote_peaks.argtypes = [p, u32, p, u64, p, p, p, u32, p, p, p]
         lib.hough_jets.argtypes = [p, u32, p, p, f32, f32, u32, p, p, p, p, p]
         lib.hough_trigger_host.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, p, p, p, p, p, p, p]
         lib.hough_status.argtypes = [p, C.POINTER(u32)]
@@ -115,16 +119,18 @@ class Hough:
     def __init__(self, n_phi0: int, n_kappa: int, n_d0: int = 1, kappa_max: float = 0.3e-3 * 3.8,
                  d0_min: float = 0.0, d0_max: float = 0.0, b_tesla: float = 3.8, n_layers: int = 8,
                  max_events: int = 1, max_hits: int = 1 << 16, max_peaks_per_event: int = 4096,
-                 max_jets_per_event: int = 256, host_chunk_events: int = 0):
+                 max_jets_per_event: int = 256, host_chunk_events: int = 0, max_candidates_per_event: int = 0):
         self.lib = load_library()
         self.cfg = HoughConfig(n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, n_layers, max_events,
-                               max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events)
+                               max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events,
+                               max_candidates_per_event)
         self._ctx = C.c_void_p()
         _check(self.lib.hough_create(C.byref(self.cfg), C.byref(self._ctx)), "hough_create")
 
     @classmethod
     def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
-                     host_chunk_events: int = 0, max_peaks: Optional[int] = None) -> "Hough":
+                     host_chunk_events: int = 0, max_peaks: Optional[int] = None,
+                     max_candidates: int = 0) -> "Hough":
         ne = w.n_events if max_events is None else max_events
         if max_hits is None:
             raise ValueError("for_workload: pass max_hits (the hit count of the largest batch per call); the context "
@@ -132,7 +138,7 @@ class Hough:
         mh = max_hits
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
                    min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
-                   host_chunk_events)
+                   host_chunk_events, max_candidates)
 
     # -- lifetime ---------------------------------------------------------------------------------
     def close(self):
@@ -181,6 +187,12 @@ class Hough:
     def hough_peaks(self, n_events, d_count, d_mask, l_min, d_peaks, d_n_peaks, stream=None):
         _check(self.lib.hough_peaks(self._ctx, n_events, _dptr(d_count), _dptr(d_mask), l_min, _dptr(d_peaks),
                                     _dptr(d_n_peaks), _stream_ptr(stream)), "hough_peaks")
+
+    def hough_vote_peaks(self, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, l_min, d_peaks, d_n_peaks,
+                         stream=None):
+        _check(self.lib.hough_vote_peaks(self._ctx, n_events, _dptr(d_hit_offsets), n_hits_total, _dptr(d_r),
+                                         _dptr(d_phi), _dptr(d_layer), l_min, _dptr(d_peaks), _dptr(d_n_peaks),
+                                         _stream_ptr(stream)), "hough_vote_peaks")
 
     def hough_jets(self, n_events, d_peaks, d_n_peaks, cone_rad, d0_cut_mm, n_displaced_min, d_tracks, d_jets,
                    d_n_jets, d_flag, stream=None):

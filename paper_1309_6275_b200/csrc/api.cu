@@ -39,6 +39,7 @@ void free_all(hough_ctx* c)
     cudaFree(c->d_rec); cudaFree(c->d_rec_u); cudaFree(c->d_key); cudaFree(c->d_seg); cudaFree(c->d_btab);
     cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
+    cudaFree(c->d_cand); cudaFree(c->d_cand_n); cudaFree(c->d_sortkeys);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
     cudaFree(c->d_hp_jets); cudaFree(c->d_hp_npeaks); cudaFree(c->d_hp_njets); cudaFree(c->d_hp_flag);
@@ -60,6 +61,7 @@ bool config_ok(const hough_config* g)
     if (g->max_hits < 1 || g->max_hits > 0xffffffffull) return false;
     if (g->max_peaks_per_event < 1 || g->max_jets_per_event < 1) return false;
     if (g->host_chunk_events > g->max_events) return false;
+    if (g->max_candidates_per_event > (1u << 24)) return false;
     return true;
 }
 
@@ -140,10 +142,22 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
     A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
     A(dev_alloc(&c->d_jetkeys, (size_t)cfg->max_events * cfg->max_peaks_per_event));
+    // fused vote -> peaks: candidate buffers for the events of one fused launch
+    c->fused_events = cfg->host_chunk_events ? cfg->host_chunk_events : cfg->max_events;
+    {
+        uint64_t cap = cfg->max_candidates_per_event;
+        if (cap == 0) { cap = 4ull * cfg->max_peaks_per_event; if (cap < 4096) cap = 4096; if (cap > (1u << 24)) cap = 1u << 24; }
+        c->cand_cap = (uint32_t)cap;
+        c->cand_cap_pow2 = 1;
+        while (c->cand_cap_pow2 < c->cand_cap) c->cand_cap_pow2 <<= 1;
+    }
+    A(dev_alloc(&c->d_cand, (size_t)c->fused_events * c->cand_cap));
+    A(dev_alloc(&c->d_cand_n, c->fused_events));
+    A(dev_alloc(&c->d_sortkeys, (size_t)c->fused_events * c->cand_cap_pow2));
     if (cfg->host_chunk_events > 0) {
         const size_t E = cfg->max_events, H = cfg->max_hits;
-        A(dev_alloc(&c->d_hp_count, (size_t)cfg->host_chunk_events * bins));
-        A(dev_alloc(&c->d_hp_mask, (size_t)cfg->host_chunk_events * bins));
+        A(dev_alloc(&c->d_hp_count, bins));                    // one event: the fallback of hough_trigger_host
+        A(dev_alloc(&c->d_hp_mask, bins));
         A(dev_alloc(&c->d_hp_off, E + 1)); A(dev_alloc(&c->d_hp_r, H)); A(dev_alloc(&c->d_hp_phi, H));
         A(dev_alloc(&c->d_hp_layer, H));
         A(dev_alloc(&c->d_hp_peaks, E * cfg->max_peaks_per_event));
@@ -167,6 +181,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
     A(cudaMemset(c->d_status, 0, 8));
     A(cudaMemset(c->d_tilectr, 0, 8));
+    A(cudaMemset(c->d_cand_n, 0, (size_t)c->fused_events * 4));
     if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
     *out = c;
     return HOUGH_OK;
@@ -212,6 +227,24 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     CK(launch_peaks(ctx, n_events, d_count, d_mask, l_min, d_peaks, d_n_peaks, st), "peak kernels");
+    return HOUGH_OK;
+}
+
+int hough_vote_peaks(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets, uint64_t n_hits_total,
+                     const float* d_r, const float* d_phi, const uint8_t* d_layer, uint32_t l_min, hough_peak* d_peaks,
+                     uint32_t* d_n_peaks, void* stream)
+{
+    if (!ctx || !d_hit_offsets || !d_peaks || !d_n_peaks) return HOUGH_EINVAL;
+    if (n_hits_total > 0 && (!d_r || !d_phi || !d_layer)) return HOUGH_EINVAL;
+    if (n_events > ctx->cfg.max_events || n_events > ctx->fused_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
+    if (l_min < 1 || l_min > ctx->cfg.n_layers) return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    if (n_events == 0) return HOUGH_OK;
+    CK(launch_prep(ctx, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, st), "hit preparation");
+    CK(launch_vote_fused(ctx, 0, n_events, l_min, st), "fused vote kernel");
+    CK(launch_recount(ctx, 0, n_events, st), "recount kernel");
+    CK(launch_peaks_finalize(ctx, n_events, d_peaks, d_n_peaks, st), "peak ordering kernel");
     return HOUGH_OK;
 }
 
@@ -274,10 +307,11 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
         const uint32_t ne = (n_events - e0 < g.host_chunk_events) ? n_events - e0 : g.host_chunk_events;
         cudaEvent_t* t = ms_stage ? &ctx->ev_pool[4 * chunk_i] : nullptr;
         if (ms_stage) cudaEventRecord(t[0], st);
-        CK(launch_vote(ctx, e0, ne, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel");
+        CK(launch_vote_fused(ctx, e0, ne, l_min, st), "fused vote kernel");
         if (ms_stage) cudaEventRecord(t[1], st);
-        CK(launch_peaks(ctx, ne, ctx->d_hp_count, ctx->d_hp_mask, l_min, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event,
-                        ctx->d_hp_npeaks + e0, st), "peak kernels");
+        CK(launch_recount(ctx, e0, ne, st), "recount kernel");
+        CK(launch_peaks_finalize(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, st),
+           "peak ordering kernel");
         if (ms_stage) cudaEventRecord(t[2], st);
         CK(launch_jets(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, cone_bins,
                        d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e0 * g.max_peaks_per_event,
@@ -286,6 +320,20 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
         if (ms_stage) cudaEventRecord(t[3], st);
     }
     CK(cudaMemcpyAsync(h_n_peaks, ctx->d_hp_npeaks, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks");
+    CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
+    // events whose candidates did not fit the buffer: the accumulator path, one event at a time, on the context's
+    // one-event planes (the prepared hits of the whole batch are still in the workspace)
+    for (uint32_t e = 0; e < n_events; ++e) {
+        if (h_n_peaks[e] != HOUGH_N_PEAKS_OVERFLOW) continue;
+        CK(launch_vote(ctx, e, 1, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel (fallback)");
+        CK(launch_peaks(ctx, 1, ctx->d_hp_count, ctx->d_hp_mask, l_min, ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event,
+                        ctx->d_hp_npeaks + e, st), "peak kernels (fallback)");
+        CK(launch_jets(ctx, 1, ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event, ctx->d_hp_npeaks + e, cone_bins,
+                       d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e * g.max_peaks_per_event,
+                       ctx->d_hp_jets + (size_t)e * g.max_jets_per_event, ctx->d_hp_njets + e, ctx->d_hp_flag + e, st),
+           "jet kernel (fallback)");
+        CK(cudaMemcpyAsync(h_n_peaks + e, ctx->d_hp_npeaks + e, 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks (fallback)");
+    }
     CK(cudaMemcpyAsync(h_n_jets, ctx->d_hp_njets, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_jets");
     CK(cudaMemcpyAsync(h_flag, ctx->d_hp_flag, (size_t)n_events, cudaMemcpyDeviceToHost, st), "D2H flag");
     if (h_peaks)

@@ -21,6 +21,10 @@ struct TileWin { int a0, len0, a1, len1; };
 // per event: start of the 16 layer segments and of the wild segment in the sorted records, then the end
 constexpr int kSegStride = HOUGH_MAX_LAYERS + 2;
 
+// Fused path: one peak candidate found in a vote tile.  cm = count | mask << 16; need = neighbour columns the tile
+// could not check, bit (dd+1)*3 + (dp+1); state = 0 pending the recount, 1 confirmed peak, 2 rejected.
+struct PeakCand { uint32_t lin, cm, need, state; };
+
 struct VotePlan {
     int k_lane;                      // KL: rows per lane; a tile has 32 * KL rows
     int tile_w;                      // phi0 columns per tile (8 in 3D, 32 * KL in 2D)
@@ -63,6 +67,12 @@ struct hough_ctx {
     uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
     uint16_t* d_grpcnt;                       // [max_events][ceil(bins/256)] peaks per group of 256 / 512 bins
     uint64_t* d_jetkeys;                      // [max_events][max_peaks]
+    // fused vote -> peaks
+    uint32_t fused_events;                    // events per fused launch the buffers below are sized for
+    uint32_t cand_cap, cand_cap_pow2;         // candidates per event (cfg.max_candidates_per_event or its default)
+    PeakCand* d_cand;                         // [fused_events][cand_cap]
+    uint32_t* d_cand_n;                       // [fused_events], zero between calls
+    unsigned long long* d_sortkeys;           // [fused_events][cand_cap_pow2] sort scratch for events beyond the SMEM sort
     // host path
     uint16_t* d_hp_count; uint16_t* d_hp_mask;     // [host_chunk_events][bins]
     uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
@@ -86,6 +96,10 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
 cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
                         int cone_bins, float d0_cut, uint32_t n_min, hough_track* d_tracks, hough_jet* d_jets,
                         uint32_t* d_n_jets, uint8_t* d_flag, cudaStream_t st);
+cudaError_t launch_vote_fused(hough_ctx* c, uint32_t first_event, uint32_t n_events, uint32_t l_min, cudaStream_t st);
+cudaError_t launch_recount(hough_ctx* c, uint32_t first_event, uint32_t n_events, cudaStream_t st);
+cudaError_t launch_peaks_finalize(hough_ctx* c, uint32_t n_events, hough_peak* d_peaks, uint32_t* d_n_peaks,
+                                  cudaStream_t st);
 cudaError_t plan_vote(hough_ctx* c);
 cudaError_t plan_peaks(hough_ctx* c);
 cudaError_t run_div_check(uint64_t n_pairs, uint64_t seed, float kmax, int nk, unsigned long long* host_out3);

@@ -37,7 +37,8 @@ __global__ void __launch_bounds__(128) jets_kernel(const JetParams p)
     const int lane = threadIdx.x & 31;
     const uint32_t e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (e >= p.n_events) return;
-    const uint32_t T = min(p.n_peaks[e], p.max_peaks);
+    const uint32_t np_e = p.n_peaks[e];
+    const uint32_t T = (np_e == HOUGH_N_PEAKS_OVERFLOW) ? 0u : min(np_e, p.max_peaks);   // overflowed fused event: no tracks
     const hough_peak* pk = p.peaks + (size_t)e * p.max_peaks;
     hough_track* trk = p.tracks + (size_t)e * p.max_peaks;
     hough_jet* jets = p.jets + (size_t)e * p.max_jets;

@@ -323,6 +323,93 @@ __global__ void __launch_bounds__(kCompactThreads) peak_compact_kernel(const uin
     if (tid == 0) n_peaks[e] = running;
 }
 
+// ---- fused path: order the confirmed candidates of an event ------------------------------------------------
+// One block per event.  The confirmed candidates (state == 1) are compacted into 64-bit keys lin << 32 | cm, sorted
+// ascending with a bitonic network (in shared memory up to kSortSmemKeys keys, in the context's global scratch
+// beyond), and the first max_peaks are written as hough_peak records; n_peaks is the true total.  An event whose
+// candidates did not fit the candidate buffer gets n_peaks = HOUGH_N_PEAKS_OVERFLOW and raises the sticky bit.
+// The event's candidate counter is reset for the next call.
+
+constexpr int kFinalThreads = 1024;
+constexpr uint32_t kSortSmemKeys = 16384;                       // 128 KB of dynamic shared memory
+
+__global__ void __launch_bounds__(kFinalThreads) peaks_finalize_kernel(const PeakCand* __restrict__ cand,
+                                                                       uint32_t* __restrict__ cand_n, uint32_t cap,
+                                                                       unsigned long long* __restrict__ gkeys,
+                                                                       uint32_t cap_pow2, uint32_t max_peaks,
+                                                                       hough_peak* __restrict__ peaks,
+                                                                       uint32_t* __restrict__ n_peaks,
+                                                                       uint32_t* __restrict__ status)
+{
+    extern __shared__ unsigned long long skeys[];
+    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_total;
+    const uint32_t e = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t n_raw = cand_n[e];
+    const uint32_t n = min(n_raw, cap);
+    const PeakCand* ce = cand + (size_t)e * cap;
+    unsigned long long* keys = (n <= kSortSmemKeys) ? skeys : gkeys + (size_t)e * cap_pow2;
+    uint32_t running = 0;
+    for (uint32_t base = 0; base < n; base += kFinalThreads) {
+        const uint32_t idx = base + (uint32_t)tid;
+        bool alive = false;
+        unsigned long long key = 0;
+        if (idx < n) {
+            const PeakCand pc = ce[idx];
+            alive = pc.state == 1u;
+            key = ((unsigned long long)pc.lin << 32) | pc.cm;
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, alive);
+        if (lane == 0) s_warp[warp] = (uint32_t)__popc(bal);
+        __syncthreads();
+        if (warp == 0) {
+            const uint32_t wsum = s_warp[lane];
+            uint32_t winc = wsum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, winc, d);
+                if (lane >= d) winc += t;
+            }
+            s_warp[lane] = winc - wsum;
+            if (lane == 31) s_total = winc;
+        }
+        __syncthreads();
+        if (alive) keys[running + s_warp[warp] + (uint32_t)__popc(bal & ((1u << lane) - 1u))] = key;
+        running += s_total;
+        __syncthreads();
+    }
+    uint32_t m = 1;
+    while (m < running) m <<= 1;
+    for (uint32_t i = running + (uint32_t)tid; i < m; i += kFinalThreads) keys[i] = ~0ull;
+    __syncthreads();
+    for (uint32_t k = 2; k <= m; k <<= 1)
+        for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+            for (uint32_t i = (uint32_t)tid; i < m; i += kFinalThreads) {
+                const uint32_t x = i ^ j;
+                if (x > i) {
+                    const unsigned long long a = keys[i], b = keys[x];
+                    if ((a > b) == ((i & k) == 0u)) { keys[i] = b; keys[x] = a; }
+                }
+            }
+            __syncthreads();
+        }
+    hough_peak* out = peaks + (size_t)e * max_peaks;
+    const uint32_t n_out = min(running, max_peaks);
+    for (uint32_t i = (uint32_t)tid; i < n_out; i += kFinalThreads) {
+        const unsigned long long key = keys[i];
+        hough_peak pk;
+        pk.lin = (uint32_t)(key >> 32); pk.count = (uint16_t)(key & 0xffffu); pk.mask = (uint16_t)((key >> 16) & 0xffffu);
+        out[i] = pk;
+    }
+    if (tid == 0) {
+        const bool over = n_raw > cap;
+        n_peaks[e] = over ? HOUGH_N_PEAKS_OVERFLOW : running;
+        if (over) atomicOr(status, (uint32_t)HOUGH_ST_CANDIDATE_OVERFLOW);
+        cand_n[e] = 0u;
+    }
+}
+
 }  // namespace
 
 cudaError_t plan_peaks(hough_ctx* c)
@@ -367,6 +454,20 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
     peak_compact_kernel<<<n_events, kCompactThreads, 0, st>>>(d_count, d_mask, c->d_bitmap, c->d_grpcnt, p.bins,
                                                               p.groups, 32u * (uint32_t)ub,
                                                               c->cfg.max_peaks_per_event, d_peaks, d_n_peaks);
+    ++c->launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_peaks_finalize(hough_ctx* c, uint32_t n_events, hough_peak* d_peaks, uint32_t* d_n_peaks,
+                                  cudaStream_t st)
+{
+    if (n_events == 0) return cudaSuccess;
+    const size_t smem = (size_t)kSortSmemKeys * sizeof(unsigned long long);
+    cudaError_t err = cudaFuncSetAttribute(peaks_finalize_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    peaks_finalize_kernel<<<n_events, kFinalThreads, smem, st>>>(c->d_cand, c->d_cand_n, c->cand_cap, c->d_sortkeys,
+                                                                 c->cand_cap_pow2, c->cfg.max_peaks_per_event, d_peaks,
+                                                                 d_n_peaks, c->d_status);
     ++c->launches;
     return cudaGetLastError();
 }
