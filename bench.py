@@ -1,20 +1,29 @@
 #!/usr/bin/env python
 """bench.py -- whole hot path (vote -> peaks -> tracks -> jets) on synthetic trigger batches, one JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3] [--events E] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3|C2|C1] [--events E]
+                  [--path fused|planes] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one batch (BASELINE.json configs[4] by default: 4,096 events,
-12-layer tracker, 128 x 1024 x 512 accumulator per event, processed in chunks of --chunk events).  `value` is
-whole-job events/s with the hits already resident in HBM; `e2e` is the same metric through hough_trigger_host
-with pinned HOST buffers (H2D of the hits and D2H of the per-event results inside the timed region).  N > 1:
-one rank per GPU (torchrun), every rank processes its own batch of the same size (weak scaling, no data-path
-collective -- events are independent); time = max over ranks, value = all ranks' events / that time.
+12-layer tracker, 128 x 1024 x 512 accumulator per event, processed in launches of --chunk events).  The default
+path is the fused one (hough_vote_peaks + hough_jets: peaks are found while the accumulator tile is in shared memory,
+no planes in HBM); --path planes times hough_vote + hough_peaks + hough_jets on accumulator planes instead, and a short
+leg of it is measured in every run for the stencil's roofline.  `value` is whole-job events/s with the hits already
+resident in HBM; `e2e` is the same metric through hough_trigger_host with pinned HOST buffers (H2D of the hits and
+D2H of n_peaks / n_jets / flag / jets inside the timed region).
+
+N > 1: one rank per GPU.  `python bench.py --gpus N` re-executes itself under torch.distributed.run when it was not
+launched by it; every rank processes its own batch of the same size (weak scaling: events are independent, no
+data-path collective), the per-event flags are all_gathered once per step (the only exchange),
+time = max over ranks, value = all ranks' events / that time.
 
 --impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample per step.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import glob
 import json
 import os
 import subprocess
@@ -28,15 +37,20 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# FP32-pipe instructions per vote of the normative O-2 sequence in scalar form: 3D = t, a, b,
-# den, the 6 FMA-pipe instructions of the IEEE division, v, u, the floor add + the per-hit m1, m2, s, rs, r2 shared by
-# the rows of a lane; 2D = m1, m2, s, division, v, u, floor.  (The kernel issues them two per instruction.)
-I_FP32 = {"3d": 15.0, "2d": 15.0}
+# FP32 (FMA-pipe) instructions per vote of the normative O-2 sequence written plainly: FADD / FMUL / FFMA in the SASS
+# of the stand-alone function csrc/o2_count.cu (IEEE division = 5 FFMA + MUFU.RCP + FCHK; the compares, F2I, MUFU and
+# FCHK run on other pipes and are not counted).  tests/test_abi_and_host.py::test_o2_instruction_count recounts them
+# from the SASS; profiles/r02_o2_sass_count.md holds the listing.  (Round 1 used a hand count of 15.)
+I_FP32 = {"3d": 17.0, "2d": 11.0}
+# the same with the five per-(hit, column) operations of 3D (m1, m2, s, rs, r2) taken as shared by the d0 bins of the
+# column (SURVEY.md 8(d) counts them "per (hit, ip)"): a stricter denominator, reported next to the contract's
+I_FP32_SHARED = {"3d": 12.0, "2d": 11.0}
 SM_COUNT, FP32_LANES = 148, 128
+SMEM_RED_PER_CLK = 32                                         # conflict-free 32-bit shared reductions per clock and SM
 
 
 # ----------------------------------------------------------------------------------------------------
-# multi-GPU helpers (also exercised by the world_size-2 gloo test)
+# multi-GPU helpers (exercised on CPU by the world_size-2 gloo test)
 # ----------------------------------------------------------------------------------------------------
 
 def shard_range(n_items: int, rank: int, world: int):
@@ -46,12 +60,15 @@ def shard_range(n_items: int, rank: int, world: int):
     return lo, lo + base + (1 if rank < rem else 0)
 
 
+def _dist_dev(dist):
+    return "cuda" if dist.get_backend() == "nccl" else "cpu"
+
+
 def max_over_ranks(x: float, dist=None) -> float:
     if dist is None or not dist.is_initialized():
         return x
     import torch
-    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
-    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    t = torch.tensor([x], dtype=torch.float64, device=_dist_dev(dist))
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
 
@@ -60,10 +77,38 @@ def sum_over_ranks(x: float, dist=None) -> float:
     if dist is None or not dist.is_initialized():
         return x
     import torch
-    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
-    t = torch.tensor([x], dtype=torch.float64, device=dev)
+    t = torch.tensor([x], dtype=torch.float64, device=_dist_dev(dist))
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
+
+
+def first_event_of_rank(n_events_per_rank: int, rank: int) -> int:
+    """Weak scaling: rank r owns the events [r * E, (r + 1) * E) of the synthetic stream."""
+    return rank * n_events_per_rank
+
+
+def gather_event_results(flag, n_peaks, n_jets, dist=None):
+    """The one exchange of the sharded job: every rank contributes flag[E] (u8), n_peaks[E] and
+    n_jets[E] (i32) of its own events; returns the three [world, E] tensors (identical on every rank; rank r's
+    events are row r).  Without a process group the inputs come back as [1, E]."""
+    import torch
+    if dist is None or not dist.is_initialized():
+        return flag[None], n_peaks[None], n_jets[None]
+    world = dist.get_world_size()
+    outs = []
+    for t in (flag, n_peaks, n_jets):
+        g = torch.empty(world * t.numel(), dtype=t.dtype, device=t.device)      # concatenation along dim 0
+        dist.all_gather_into_tensor(g, t.contiguous().view(-1))
+        outs.append(g.view((world,) + tuple(t.shape)))
+    return tuple(outs)
+
+
+def reexec_under_torchrun(args, argv):
+    """`python bench.py --gpus N` (N > 1) without a launcher: start N ranks on this node and forward their output."""
+    port = 29500 + (os.getpid() % 2000)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + argv
+    raise SystemExit(subprocess.call(cmd))
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -122,6 +167,35 @@ def measured_peaks():
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
+def traffic_from_profiles(kernel_substr: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum (GB per launch) of the newest committed `ncu --page raw --csv`
+    export under profiles/ whose kernel name contains kernel_substr; (None, None) if there is none."""
+    best = (None, None)
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_raw.csv"))):
+        try:
+            rows = list(csv.reader(open(path, newline="")))
+        except Exception:
+            continue
+        if len(rows) < 3:
+            continue
+        head, units = rows[0], rows[1]
+        try:
+            i_name = head.index("Kernel Name")
+            i_r, i_w = head.index("dram__bytes_read.sum"), head.index("dram__bytes_write.sum")
+        except ValueError:
+            continue
+        scale = {"byte": 1e-9, "Kbyte": 1e-6, "Mbyte": 1e-3, "Gbyte": 1.0, "Tbyte": 1e3}
+        for row in rows[2:]:
+            if kernel_substr in row[i_name]:
+                try:
+                    gb = float(row[i_r].replace(",", "")) * scale[units[i_r]] + \
+                         float(row[i_w].replace(",", "")) * scale[units[i_w]]
+                except Exception:
+                    continue
+                best = (gb, os.path.basename(path))
+    return best
+
+
 # ----------------------------------------------------------------------------------------------------
 # workloads
 # ----------------------------------------------------------------------------------------------------
@@ -156,7 +230,7 @@ def cpu_oracle_rate(w, batch, budget_s: float = 15.0):
 
 
 # ----------------------------------------------------------------------------------------------------
-# the two arms
+# the reference arm = the oracle
 # ----------------------------------------------------------------------------------------------------
 
 def run_reference(args):
@@ -196,6 +270,166 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+# ----------------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------------
+
+class DeviceRun:
+    """One workload resident on the device: context, uploaded hits, output tensors, and the step function."""
+
+    def __init__(self, w, batch, chunk: int, path: str):
+        import torch
+        from paper_1309_6275_b200 import binding as B
+        self.torch, self.B, self.w, self.batch, self.path = torch, B, w, batch, path
+        self.E = batch.n_events
+        self.chunk = min(chunk, self.E)
+        self.offs = batch.hit_offsets.astype(np.int64)
+        self.n_chunks = (self.E + self.chunk - 1) // self.chunk
+        hits_per_chunk = max(int(self.offs[min(c + self.chunk, self.E)] - self.offs[c]) for c in range(0, self.E, self.chunk))
+        self.h = B.Hough.for_workload(w, max_events=self.chunk, max_hits=max(1, hits_per_chunk))
+        self.off, self.r, self.phi, self.layer = B.upload_batch(batch)
+        self.out = self.h.alloc_outputs(self.E)
+        self.count = self.mask = None
+        if path == "planes":
+            self.count, self.mask = self.h.alloc_planes(self.chunk)
+        self.stream = torch.cuda.current_stream()
+
+    def step(self):
+        h, w, out, st = self.h, self.w, self.out, self.stream
+        for ci in range(self.n_chunks):
+            e0 = ci * self.chunk
+            ne = min(self.chunk, self.E - e0)
+            hb, he = int(self.offs[e0]), int(self.offs[e0 + ne])
+            a = (ne, self.off[e0:e0 + ne + 1], he - hb, self.r[hb:he], self.phi[hb:he], self.layer[hb:he])
+            if self.path == "fused":
+                h.hough_vote_peaks(*a, w.l_min, out["peaks"][e0:], out["n_peaks"][e0:], st)
+            else:
+                h.hough_vote(*a, self.count, self.mask, st)
+                h.hough_peaks(ne, self.count, self.mask, w.l_min, out["peaks"][e0:], out["n_peaks"][e0:], st)
+            h.hough_jets(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.cone_rad, w.d0_cut_mm, w.n_displaced_min,
+                         out["tracks"][e0:], out["jets"][e0:], out["n_jets"][e0:], out["flag"][e0:], st)
+
+    def timed(self, steps: int, warmup: int, dist=None, after_step=None):
+        """(ms total, stage ms {prep, vote, peaks, jets}, launches) for `steps` steps after `warmup` untimed ones."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.step()
+            if after_step: after_step()
+        torch.cuda.synchronize()
+        if dist: dist.barrier()
+        self.h.hough_profile(True)
+        self.h.hough_profile_read()
+        l0 = self.h.hough_launch_count()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(self.stream)
+        for _ in range(steps):
+            self.step()
+            if after_step: after_step()
+        b.record(self.stream)
+        torch.cuda.synchronize()
+        if dist: dist.barrier()
+        stage, _ = self.h.hough_profile_read()
+        self.h.hough_profile(False)
+        return a.elapsed_time(b), stage, self.h.hough_launch_count() - l0
+
+    def close(self):
+        self.count = self.mask = None
+        self.h.close()
+
+
+def count_votes(w, batch, sub: int = 16):
+    """Votes of the batch = sum of the count planes (untimed; accumulator path on `sub` events at a time)."""
+    import torch
+    from paper_1309_6275_b200 import binding as B
+    E = batch.n_events
+    sub = max(1, min(sub, E, int(8.6e9 // (4 * w.bins_per_event)) or 1))
+    offs = batch.hit_offsets.astype(np.int64)
+    hits = max(int(offs[min(c + sub, E)] - offs[c]) for c in range(0, E, sub))
+    h = B.Hough.for_workload(w, max_events=sub, max_hits=max(1, hits))
+    off, r, phi, layer = B.upload_batch(batch)
+    count, mask = h.alloc_planes(sub)
+    total = 0
+    for e0 in range(0, E, sub):
+        ne = min(sub, E - e0)
+        hb, he = int(offs[e0]), int(offs[e0 + ne])
+        h.hough_vote(ne, off[e0:e0 + ne + 1], he - hb, r[hb:he], phi[hb:he], layer[hb:he], count, mask)
+        total += int((count[:ne].to(torch.int32) & 0xFFFF).sum(dtype=torch.int64).item())
+    h.close()
+    del count, mask
+    torch.cuda.empty_cache()
+    return float(total)
+
+
+def vote_roofline(mode, votes, bins_written, ms_vote, launches, hbm_gbs, sm_max_mhz, peak_src, kernel, traffic=None):
+    """Roofline of the vote kernel: max of the FP32 term (I_FP32 instructions per vote on 148 x 128 lanes), the
+    shared-reduction term (2 per vote at 32 per clock and SM) and -- accumulator path only -- the HBM-write term
+    (4 B per bin)."""
+    s = ms_vote * 1e-3
+    clk = sm_max_mhz * 1e6
+    fp32_peak = SM_COUNT * FP32_LANES * clk
+    red_peak = SM_COUNT * SMEM_RED_PER_CLK * clk
+    t_fp32 = votes * I_FP32[mode] / fp32_peak
+    t_red = 2.0 * votes / red_peak
+    t_hbm = 4.0 * bins_written / (hbm_gbs * 1e9)
+    terms = {"fp32": t_fp32 * 1e3, "shared_reductions": t_red * 1e3, "hbm_write": t_hbm * 1e3}
+    if t_hbm >= max(t_fp32, t_red):
+        ach = 4.0 * bins_written / s / 1e9
+        rl = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs}
+    else:
+        ach = votes * I_FP32[mode] / s
+        rl = {"bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12, "unit": "Tinstr/s",
+              "frac": ach / fp32_peak}
+    rl.update({"traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
+               "kernel": kernel, "ms_per_launch": ms_vote / max(1, launches), "launches": launches,
+               "i_fp32_per_vote": I_FP32[mode], "t_bound_terms_ms": terms,
+               "frac_fp32_shared_hit_terms": votes * I_FP32_SHARED[mode] / s / fp32_peak,
+               "peak_source": peak_src + "; FP32 peak = 148 SM x 128 lanes x sm_max clock (no FMA credit)",
+               "note": "duration = CUDA events around the vote kernel alone (hough_profile, launching stream)"})
+    return rl
+
+
+def stencil_roofline(bins_read, ms_peaks, launches, hbm_gbs):
+    ach = 2.0 * bins_read / (ms_peaks * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": "peak_stencil_kernel+peak_compact_kernel", "achieved": ach, "peak": hbm_gbs,
+            "unit": "GB/s", "frac": ach / hbm_gbs, "traffic": None, "ms_per_launch": ms_peaks / max(1, launches),
+            "launches": launches}
+
+
+def measure_config(name: str, hbm_gbs, sm_max_mhz, peak_src, steps: int = 3):
+    """Short device-resident measurement of one of the other configs for the per_config block."""
+    import torch
+    from paper_1309_6275_b200 import workloads as W
+    w = make_workload(name, None)
+    batch = W.generate(w)
+    mode = "3d" if w.n_d0 > 1 else "2d"
+    chunk = max(1, min(w.n_events, int(34.4e9 // (4 * w.bins_per_event))))
+    res = {"events": w.n_events, "hits": batch.n_hits, "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min}
+    votes = count_votes(w, batch)
+    res["votes"] = votes
+    single = w.n_events == 1
+    reps = 200 if single else steps
+    for path in ("fused", "planes"):
+        run = DeviceRun(w, batch, chunk, path)
+        ms, stage, launches = run.timed(reps, 20 if single else 2)
+        n_launch = reps * run.n_chunks
+        d = {"ms_per_step": ms / reps, "events_per_sec": w.n_events * reps / (ms * 1e-3),
+             "stage_ms_per_step": {k: v / reps for k, v in zip(("prep", "vote", "peaks", "jets"), stage)},
+             "launches_per_step": launches // reps}
+        if single:
+            d["latency_us"] = 1e3 * ms / reps
+        else:
+            bins_w = 0 if path == "fused" else w.bins_per_event * w.n_events * reps
+            d["roofline"] = vote_roofline(mode, votes * reps, bins_w, stage[1], n_launch, hbm_gbs, sm_max_mhz, peak_src,
+                                          "vote_kernel<fused>" if path == "fused" else "vote_kernel")
+            if path == "planes":
+                d["roofline_stencil"] = stencil_roofline(w.bins_per_event * w.n_events * reps, stage[2], n_launch, hbm_gbs)
+        res[path] = d
+        run.close()
+        torch.cuda.empty_cache()
+    return res
+
+
 def run_ours(args):
     import torch
     from paper_1309_6275_b200 import binding as B
@@ -204,6 +438,9 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; launch one rank per GPU "
+                         f"(python bench.py --gpus N starts them itself)")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
     torch.cuda.set_device(local)
@@ -214,99 +451,85 @@ def run_ours(args):
 
     w = make_workload(args.workload, args.events)
     E = w.n_events
-    # events per vote/peaks/jets launch: --chunk, else as many as fit in about 34 GB of planes (C5: 128 events)
+    # events per launch: --chunk, else as many as would fit in about 34 GB of planes (C5: 128 events)
     chunk = args.chunk if args.chunk > 0 else max(1, int(34.4e9 // (4 * w.bins_per_event)))
     chunk = min(chunk, E)
     mode = "3d" if w.n_d0 > 1 else "2d"
-    # weak scaling: every rank owns a batch of E events (event indices continue across ranks)
-    batch = W.generate(w, E, first_event=rank * E)
+    batch = W.generate(w, E, first_event=first_event_of_rank(E, rank))      # weak scaling: every rank its own events
     H = batch.n_hits
     bins = w.bins_per_event
+    hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
 
-    h = B.Hough.for_workload(w, max_events=chunk, max_hits=H)
-    offs = batch.hit_offsets.astype(np.int64)
-    off, r, phi, layer = B.upload_batch(batch)
-    count, mask = h.alloc_planes(chunk)
-    out = h.alloc_outputs(E)
-    stream = torch.cuda.current_stream()
-    n_chunks = (E + chunk - 1) // chunk
-    ev = lambda: torch.cuda.Event(enable_timing=True)
+    votes_per_step = count_votes(w, batch)
 
-    def one_step(stage_events=None, votes_acc=None):
-        for ci in range(n_chunks):
-            e0 = ci * chunk
-            ne = min(chunk, E - e0)
-            t = [ev() for _ in range(4)] if stage_events is not None else None
-            if t: t[0].record(stream)
-            hb, he = int(offs[e0]), int(offs[e0 + ne])
-            h.hough_vote(ne, off[e0:e0 + ne + 1], he - hb, r[hb:he], phi[hb:he], layer[hb:he], count, mask, stream)
-            if t: t[1].record(stream)
-            h.hough_peaks(ne, count, mask, w.l_min, out["peaks"][e0:], out["n_peaks"][e0:], stream)
-            if t: t[2].record(stream)
-            h.hough_jets(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.cone_rad, w.d0_cut_mm, w.n_displaced_min,
-                         out["tracks"][e0:], out["jets"][e0:], out["n_jets"][e0:], out["flag"][e0:], stream)
-            if t:
-                t[3].record(stream)
-                stage_events.append(t)
-            if votes_acc is not None:
-                votes_acc.append(int((count[:ne].to(torch.int32) & 0xFFFF).sum(dtype=torch.int64).item()))
+    run = DeviceRun(w, batch, chunk, args.path)
+    gathered = {}
 
-    # warm-up (the first warm-up step also counts the votes, untimed)
-    votes_chunks = []
-    for i in range(args.warmup):
-        one_step(votes_acc=votes_chunks if i == 0 else None)
-    if not votes_chunks:
-        one_step(votes_acc=votes_chunks)
-    votes_per_step = float(sum(votes_chunks))
-    torch.cuda.synchronize()
-    if dist: dist.barrier()
+    def exchange():
+        if dist is not None:
+            gathered["v"] = gather_event_results(run.out["flag"], run.out["n_peaks"], run.out["n_jets"], dist)
 
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.3)
-    launches0 = h.hough_launch_count()
-    stage_events = []
-    t_start, t_stop = ev(), ev()
-    torch.cuda.synchronize()
     wall0 = time.time()
-    t_start.record(stream)
-    for _ in range(args.steps):
-        one_step(stage_events=stage_events)
-    t_stop.record(stream)
-    torch.cuda.synchronize()
+    ms_total, stage, launches = run.timed(args.steps, args.warmup, dist, exchange if dist else None)
     wall1 = time.time()
-    if dist: dist.barrier()
-    ms_total = t_start.elapsed_time(t_stop)
-    clocks = sampler.stop(wall0, wall1)
-    launches = h.hough_launch_count() - launches0
-    status = h.hough_status()
-
-    ms_vote = sum(t[0].elapsed_time(t[1]) for t in stage_events)
-    ms_peaks = sum(t[1].elapsed_time(t[2]) for t in stage_events)
-    ms_jets = sum(t[2].elapsed_time(t[3]) for t in stage_events)
-    n_flag = int(out["flag"].sum().item())
-    n_peaks_total = int(out["n_peaks"].to(torch.int64).sum().item())
+    clocks = sampler.stop(wall0 + 0.0, wall1)
+    status = run.h.hough_status()
+    n_flag = int(run.out["flag"].sum().item())
+    n_peaks_total = int(run.out["n_peaks"].to(torch.int64).sum().item())
+    flags_dev = run.out["flag"].cpu().numpy().copy()
+    npk_dev = run.out["n_peaks"].cpu().numpy().copy()
+    job_flags = None
+    if dist is not None:
+        gf = gathered["v"][0]
+        assert gf.shape == (world, E) and bool((gf[rank] == run.out["flag"]).all())
+        job_flags = int(gf.sum().item())
 
     ms_max = max_over_ranks(ms_total, dist)
     total_events = sum_over_ranks(float(E * args.steps), dist)
     value = total_events / (ms_max * 1e-3)
+    n_launch = args.steps * run.n_chunks
+    run.close()
+    torch.cuda.empty_cache()
+
+    # ---- the accumulator path on a short leg (stencil roofline; vote kernel with the plane flush) ----
+    planes = None
+    if rank == 0 and args.path == "fused" and not args.no_planes_leg:
+        n_ev = min(E, 2 * chunk)
+        sub = batch.slice(0, n_ev)
+        votes_sub = votes_per_step * (sub.n_hits / max(1, H))             # (estimate only used if it binds: it does not at C5/C3)
+        prun = DeviceRun(w, sub, chunk, "planes")
+        p_steps = 3
+        p_ms, p_stage, p_launches = prun.timed(p_steps, 1)
+        pl = p_steps * prun.n_chunks
+        planes = {"events": n_ev, "ms_per_step": p_ms / p_steps, "events_per_sec": n_ev * p_steps / (p_ms * 1e-3),
+                  "stage_ms_per_step": {k: v / p_steps for k, v in zip(("prep", "vote", "peaks", "jets"), p_stage)},
+                  "roofline_vote": vote_roofline(mode, votes_sub * p_steps, bins * n_ev * p_steps, p_stage[1], pl, hbm_gbs,
+                                                 sm_max_mhz, peak_src, "vote_kernel"),
+                  "roofline_stencil": stencil_roofline(bins * n_ev * p_steps, p_stage[2], pl, hbm_gbs)}
+        same = bool(np.array_equal(prun.out["flag"].cpu().numpy(), flags_dev[:n_ev]) and
+                    np.array_equal(prun.out["n_peaks"].cpu().numpy(), npk_dev[:n_ev]))
+        planes["matches_fused_path"] = same
+        prun.close()
+        torch.cuda.empty_cache()
 
     # ---- e2e: the same batch through hough_trigger_host with pinned host buffers ----
-    del count, mask
-    h.close()
-    torch.cuda.empty_cache()
     h2 = B.Hough.for_workload(w, max_events=E, max_hits=H, host_chunk_events=chunk)
     pin = lambda a: torch.from_numpy(a).pin_memory()
     h_off, h_r, h_phi, h_layer = pin(batch.hit_offsets.view(np.int32)), pin(batch.r), pin(batch.phi), pin(batch.layer)
     h_np = torch.zeros(E, dtype=torch.int32).pin_memory(); h_nj = torch.zeros(E, dtype=torch.int32).pin_memory()
     h_fl = torch.zeros(E, dtype=torch.uint8).pin_memory()
+    h_jets = torch.zeros((E, w.max_jets, 20), dtype=torch.uint8).pin_memory()
+    stream = torch.cuda.current_stream()
     e2e_steps = max(1, min(args.steps, 3))
     call = lambda: h2.hough_trigger_host(E, h_off, H, h_r, h_phi, h_layer, w.l_min, w.cone_rad, w.d0_cut_mm,
-                                         w.n_displaced_min, h_np, h_nj, h_fl, None, None, None, stream)
+                                         w.n_displaced_min, h_np, h_nj, h_fl, None, h_jets, None, stream)
     call()
     torch.cuda.synchronize()
     if dist: dist.barrier()
-    a, b = ev(), ev()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record(stream)
     for _ in range(e2e_steps):
         call()
@@ -314,63 +537,57 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_e2e = max_over_ranks(a.elapsed_time(b), dist)
     e2e_value = sum_over_ranks(float(E * e2e_steps), dist) / (ms_e2e * 1e-3)
-    e2e_ok = bool(np.array_equal(h_fl.numpy(), out["flag"].cpu().numpy()) and
-                  np.array_equal(h_np.numpy(), out["n_peaks"].cpu().numpy()))
+    e2e_ok = bool(np.array_equal(h_fl.numpy(), flags_dev) and np.array_equal(h_np.numpy(), npk_dev))
     h2_launches = h2.hough_launch_count()
     h2.close()
+    torch.cuda.empty_cache()
 
     if rank != 0:
         if dist: dist.destroy_process_group()
         return
 
-    hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
-    # roofline of the dominant kernel (vote): FP32-pipe bound (max of atomics / FP32 / HBM-write terms)
-    vote_s = ms_vote * 1e-3
     votes_timed = votes_per_step * args.steps
-    fp32_peak = SM_COUNT * FP32_LANES * sm_max_mhz * 1e6            # thread-instructions / s, no FMA credit
-    achieved_instr = votes_timed * I_FP32[mode] / vote_s
-    t_hbm = 4.0 * bins * E * args.steps / (hbm_gbs * 1e9)
-    t_fp32 = votes_timed * I_FP32[mode] / fp32_peak
-    bound = "alu" if t_fp32 >= t_hbm else "hbm"
-    # dram__bytes_read.sum + dram__bytes_write.sum of one vote launch (ncu --set full, profiles/r01c_summary.md);
-    # only known for the launch shape that capture was taken on (C5, 128 events per launch)
-    traffic = 34.33 if (w.name.startswith("C5") and chunk == 128) else None
-    if bound == "alu":
-        roofline = {"bound": "alu", "achieved": achieved_instr / 1e12, "peak": fp32_peak / 1e12, "unit": "Tinstr/s",
-                    "frac": achieved_instr / fp32_peak, "traffic": None}
-    else:
-        ach = 4.0 * bins * E * args.steps / vote_s / 1e9
-        roofline = {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
-                    "traffic": traffic, "traffic_unit": "GB per launch (algorithmic: %.2f)" % (4.0 * bins * chunk / 1e9)}
-    roofline.update({"kernel": "vote_kernel", "peak_source": peak_src + "; FP32 peak = 148 SM x 128 lanes x sm_max clock",
-                     "ms_per_launch": ms_vote / max(1, len(stage_events)), "launches": len(stage_events),
-                     "i_fp32_per_vote": I_FP32[mode], "t_bound_terms_ms": {"fp32": t_fp32 * 1e3, "hbm_write": t_hbm * 1e3},
-                     "note": "duration = CUDA events around hough_vote (includes the two small A0 prep kernels)"})
-    stencil_bytes = 2.0 * bins * E * args.steps
-    ach_st = stencil_bytes / (ms_peaks * 1e-3) / 1e9
-    roofline_stencil = {"bound": "hbm", "kernel": "peak_stencil_kernel+peak_compact_kernel", "achieved": ach_st,
-                        "peak": hbm_gbs, "unit": "GB/s", "frac": ach_st / hbm_gbs, "traffic": None,
-                        "ms_per_launch": ms_peaks / max(1, len(stage_events))}
+    fused = args.path == "fused"
+    kern = "vote_kernel<fused>" if fused else "vote_kernel"
+    traffic = traffic_from_profiles("vote_kernel") if (w.name == "C5" and chunk == 128) else None
+    roofline = vote_roofline(mode, votes_timed, 0 if fused else bins * E * args.steps, stage[1], n_launch, hbm_gbs,
+                             sm_max_mhz, peak_src, kern, traffic)
+
+    per_config = None
+    if not args.no_per_config and world == 1 and w.name == "C5" and not args.events:
+        per_config = {}
+        for name in ("C1", "C2", "C3", "C4"):
+            per_config[name] = measure_config(name, hbm_gbs, sm_max_mhz, peak_src)
 
     cpu = cpu_oracle_rate(w, batch) if not args.no_cpu_baseline else None
 
+    if fused:
+        l2_note = (f"no L2 flush needed: the fused path streams nothing but the hits ({H * 25 / 1e6:.0f} MB of raw + "
+                   f"prepared records per step, larger than the 126 MB L2 for C5) and is compute-bound")
+    else:
+        l2_note = f"working set >> L2: {4 * bins * chunk / 1e9:.1f} GB of planes rewritten and re-read every launch"
     line = {
         "metric": "events_per_sec", "value": value, "unit": "events/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": w.name, "events_per_gpu": E, "chunk_events": chunk, "hits": H,
-                   "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min, "cone_rad": w.cone_rad,
-                   "l2": "working set >> L2: 268 MB of planes per event, rewritten every chunk"},
+        "config": {"workload": w.name, "path": args.path, "events_per_gpu": E, "chunk_events": chunk, "hits": H,
+                   "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min, "cone_rad": w.cone_rad, "l2": l2_note},
         "votes_per_sec": votes_timed * world / (ms_max * 1e-3) if world == 1 else None,
         "votes_per_step": votes_per_step,
-        "stage_ms_per_step": {"vote": ms_vote / args.steps, "peaks": ms_peaks / args.steps, "jets": ms_jets / args.steps},
-        "events_flagged": n_flag, "peaks_total": n_peaks_total, "status_bits": status,
-        "clocks": clocks,
+        "stage_ms_per_step": {k: v / args.steps for k, v in zip(("prep", "vote", "peaks", "jets"), stage)},
+        "events_flagged": n_flag, "events_flagged_all_ranks": job_flags, "peaks_total": n_peaks_total,
+        "status_bits": status, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": int(H * 9 + (E + 1) * 4),
-                "d2h_bytes_per_step": int(E * 9), "steps": e2e_steps, "matches_device_path": e2e_ok},
+                "d2h_bytes_per_step": int(E * 9 + E * w.max_jets * 20), "steps": e2e_steps,
+                "matches_device_path": e2e_ok},
         "gpu_launches": int(launches), "gpu_launches_e2e": int(h2_launches),
-        "roofline": roofline, "roofline_stencil": roofline_stencil,
+        "roofline": roofline,
     }
+    if planes:
+        line["accumulator_path"] = planes
+        line["roofline_stencil"] = planes["roofline_stencil"]
+    if per_config:
+        line["per_config"] = per_config
     if cpu:
         line["cpu_baseline"] = cpu
     print(json.dumps(line))
@@ -384,14 +601,19 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--path", default="fused", choices=["fused", "planes"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (0 = the config's)")
-    ap.add_argument("--chunk", type=int, default=0, help="events per vote/peaks/jets launch (0: what fits in 34 GB of planes)")
+    ap.add_argument("--chunk", type=int, default=0, help="events per launch (0: what would fit in 34 GB of planes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--no-planes-leg", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    else:
-        run_ours(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        reexec_under_torchrun(args, sys.argv[1:])
+    run_ours(args)
 
 
 if __name__ == "__main__":

@@ -178,6 +178,16 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
 /* Synchronises the stream of the last call on ctx and returns (and keeps) the sticky status bits.  HOST out. */
 int hough_status(hough_ctx* ctx, uint32_t* host_status_bits);
 
+/*
+ * Per-stage device timing with CUDA events on the caller's stream (what bench.py's roofline uses).  While enabled,
+ * every call on ctx records an event before each stage and one at its end.  hough_profile_read waits for the last
+ * recorded event and returns the milliseconds accumulated since the previous read in
+ * h_ms[0..3] = {hit preparation, vote kernel, peak kernels (stencil + compaction, or recount + ordering), jets}
+ * and the number of calls seen.  HOST out.  Costs one event record (a few microseconds) per stage while enabled.
+ */
+int hough_profile(hough_ctx* ctx, int enable);
+int hough_profile_read(hough_ctx* ctx, float* h_ms /* [4] */, uint32_t* h_calls /* may be null */);
+
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches).  HOST out. */
 int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);
 

@@ -26,7 +26,7 @@ N_PEAKS_OVERFLOW = 0xFFFFFFFF
 EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_vote_peaks",
            "hough_jets",
            "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
-           "hough_debug_prepared_hits", "hough_debug_div_check"]
+           "hough_debug_prepared_hits", "hough_debug_div_check", "hough_profile", "hough_profile_read"]
 
 
 class HoughConfig(C.Structure):
@@ -70,6 +70,8 @@ def load_library() -> C.CDLL:
         lib.hough_microbench.argtypes = [C.c_int, C.c_size_t, C.POINTER(C.c_double)]
         lib.hough_debug_prepared_hits.argtypes = [p, u64, p, C.POINTER(u32)]
         lib.hough_debug_div_check.argtypes = [u64, u64, f32, u32, C.POINTER(u64)]
+        lib.hough_profile.argtypes = [p, C.c_int]
+        lib.hough_profile_read.argtypes = [p, C.POINTER(f32), C.POINTER(u32)]
         lib.hough_strerror.argtypes = [C.c_int]
         lib.hough_strerror.restype = C.c_char_p
         for name in EXPORTS:
@@ -225,6 +227,15 @@ class Hough:
         _check(self.lib.hough_debug_prepared_hits(self._ctx, n_hits, C.c_void_p(rec.ctypes.data), C.byref(risk)),
                "hough_debug_prepared_hits")
         return rec[:n_hits], risk.value
+
+    def hough_profile(self, enable: bool):
+        _check(self.lib.hough_profile(self._ctx, 1 if enable else 0), "hough_profile")
+
+    def hough_profile_read(self):
+        """(ms per stage {prep, vote, peaks, jets} since the last read, number of calls)."""
+        ms = (C.c_float * 4)(); n = C.c_uint32(0)
+        _check(self.lib.hough_profile_read(self._ctx, ms, C.byref(n)), "hough_profile_read")
+        return [float(x) for x in ms], int(n.value)
 
     def hough_launch_count(self) -> int:
         out = C.c_uint64(0)

@@ -47,6 +47,22 @@ void free_all(hough_ctx* c)
     c->ev_pool.clear();
 }
 
+// hough_profile: a mark on the stream; the interval up to the next mark of the same call is charged to `label`
+constexpr size_t kMaxProfMarks = 1u << 18;
+void prof_mark(hough_ctx* c, int label, cudaStream_t st)
+{
+    if (!c->prof_on || c->ev_used >= kMaxProfMarks) return;
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t ev = nullptr;
+        if (cudaEventCreate(&ev) != cudaSuccess) { cudaGetLastError(); return; }
+        c->ev_pool.push_back(ev);
+        c->ev_label.push_back(-1);
+    }
+    cudaEventRecord(c->ev_pool[c->ev_used], st);
+    c->ev_label[c->ev_used] = label;
+    ++c->ev_used;
+}
+
 bool config_ok(const hough_config* g)
 {
     if (g->n_phi0 < 4 || g->n_phi0 > (1u << 20)) return false;
@@ -213,8 +229,11 @@ int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets,
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     if (n_events == 0) return HOUGH_OK;
+    prof_mark(ctx, 0, st);
     CK(launch_prep(ctx, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, st), "hit preparation");
+    prof_mark(ctx, 1, st);
     CK(launch_vote(ctx, 0, n_events, d_count, d_mask, st), "vote kernel");
+    prof_mark(ctx, -1, st);
     return HOUGH_OK;
 }
 
@@ -226,7 +245,9 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
     if (((uintptr_t)d_count | (uintptr_t)d_mask) & 15u) return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
+    prof_mark(ctx, 2, st);
     CK(launch_peaks(ctx, n_events, d_count, d_mask, l_min, d_peaks, d_n_peaks, st), "peak kernels");
+    prof_mark(ctx, -1, st);
     return HOUGH_OK;
 }
 
@@ -241,10 +262,14 @@ int hough_vote_peaks(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_of
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     if (n_events == 0) return HOUGH_OK;
+    prof_mark(ctx, 0, st);
     CK(launch_prep(ctx, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, st), "hit preparation");
+    prof_mark(ctx, 1, st);
     CK(launch_vote_fused(ctx, 0, n_events, l_min, st), "fused vote kernel");
+    prof_mark(ctx, 2, st);
     CK(launch_recount(ctx, 0, n_events, st), "recount kernel");
     CK(launch_peaks_finalize(ctx, n_events, d_peaks, d_n_peaks, st), "peak ordering kernel");
+    prof_mark(ctx, -1, st);
     return HOUGH_OK;
 }
 
@@ -264,8 +289,10 @@ int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, con
     if (n_events > ctx->cfg.max_events || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm)) return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
+    prof_mark(ctx, 3, st);
     CK(launch_jets(ctx, n_events, d_peaks, d_n_peaks, cone_bins_of(cone_rad, ctx->cfg.n_phi0), d0_cut_mm,
                    n_displaced_min, d_tracks, d_jets, d_n_jets, d_flag, st), "jet kernel");
+    prof_mark(ctx, -1, st);
     return HOUGH_OK;
 }
 
@@ -291,34 +318,32 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
         CK(cudaMemcpyAsync(ctx->d_hp_phi, h_phi, n_hits_total * 4, cudaMemcpyHostToDevice, st), "H2D phi");
         CK(cudaMemcpyAsync(ctx->d_hp_layer, h_layer, n_hits_total, cudaMemcpyHostToDevice, st), "H2D layer");
     }
+    // ms_stage: the context's stage profile (hough_profile) is switched on for this call and read at its end
+    const bool prof_was_on = ctx->prof_on;
+    if (ms_stage) {
+        float drop[4]; uint32_t nc = 0;
+        if (prof_was_on) hough_profile_read(ctx, drop, &nc);     // keep earlier intervals out of this call's numbers
+        ctx->prof_on = true;
+    }
     // hits are prepared once for the whole batch; the chunks then share the prepared records
+    prof_mark(ctx, 0, st);
     CK(launch_prep(ctx, n_events, ctx->d_hp_off, n_hits_total, ctx->d_hp_r, ctx->d_hp_phi, ctx->d_hp_layer, st), "hit preparation");
     const int cone_bins = cone_bins_of(cone_rad, g.n_phi0);
-    // stage timing uses events owned by the context (created once, reused by later calls, freed in hough_destroy)
-    const size_t n_chunks = ((size_t)n_events + g.host_chunk_events - 1) / g.host_chunk_events;
-    if (ms_stage)
-        while (ctx->ev_pool.size() < 4 * n_chunks) {
-            cudaEvent_t ev = nullptr;
-            CK(cudaEventCreate(&ev), "cudaEventCreate");
-            ctx->ev_pool.push_back(ev);
-        }
-    size_t chunk_i = 0;
-    for (uint32_t e0 = 0; e0 < n_events; e0 += g.host_chunk_events, ++chunk_i) {
+    for (uint32_t e0 = 0; e0 < n_events; e0 += g.host_chunk_events) {
         const uint32_t ne = (n_events - e0 < g.host_chunk_events) ? n_events - e0 : g.host_chunk_events;
-        cudaEvent_t* t = ms_stage ? &ctx->ev_pool[4 * chunk_i] : nullptr;
-        if (ms_stage) cudaEventRecord(t[0], st);
+        prof_mark(ctx, 1, st);
         CK(launch_vote_fused(ctx, e0, ne, l_min, st), "fused vote kernel");
-        if (ms_stage) cudaEventRecord(t[1], st);
+        prof_mark(ctx, 2, st);
         CK(launch_recount(ctx, e0, ne, st), "recount kernel");
         CK(launch_peaks_finalize(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, st),
            "peak ordering kernel");
-        if (ms_stage) cudaEventRecord(t[2], st);
+        prof_mark(ctx, 3, st);
         CK(launch_jets(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, cone_bins,
                        d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e0 * g.max_peaks_per_event,
                        ctx->d_hp_jets + (size_t)e0 * g.max_jets_per_event, ctx->d_hp_njets + e0, ctx->d_hp_flag + e0, st),
            "jet kernel");
-        if (ms_stage) cudaEventRecord(t[3], st);
     }
+    prof_mark(ctx, -1, st);
     CK(cudaMemcpyAsync(h_n_peaks, ctx->d_hp_npeaks, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks");
     CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
     // events whose candidates did not fit the buffer: the accumulator path, one event at a time, on the context's
@@ -344,12 +369,10 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
                            cudaMemcpyDeviceToHost, st), "D2H jets");
     CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
     if (ms_stage) {
-        for (size_t i = 0; i < 4 * n_chunks; i += 4)
-            for (int s = 0; s < 3; ++s) {
-                float ms = 0.f;
-                cudaEventElapsedTime(&ms, ctx->ev_pool[i + s], ctx->ev_pool[i + s + 1]);
-                ms_stage[s] += ms;
-            }
+        float ms[4]; uint32_t nc = 0;
+        hough_profile_read(ctx, ms, &nc);
+        ms_stage[0] = ms[0] + ms[1]; ms_stage[1] = ms[2]; ms_stage[2] = ms[3];
+        ctx->prof_on = prof_was_on;
     }
     return HOUGH_OK;
 }
@@ -384,6 +407,31 @@ int hough_debug_div_check(uint64_t n_pairs, uint64_t seed, float kappa_max, uint
     unsigned long long out[3] = {0, 0, 0};
     CK(run_div_check(n_pairs, seed, kappa_max, (int)n_kappa, out), "division check kernel");
     for (int i = 0; i < 3; ++i) h_out[i] = out[i];
+    return HOUGH_OK;
+}
+
+int hough_profile(hough_ctx* ctx, int enable)
+{
+    if (!ctx) return HOUGH_EINVAL;
+    ctx->prof_on = enable != 0;
+    return HOUGH_OK;
+}
+
+int hough_profile_read(hough_ctx* ctx, float* h_ms, uint32_t* h_calls)
+{
+    if (!ctx || !h_ms) return HOUGH_EINVAL;
+    for (int i = 0; i < 4; ++i) h_ms[i] = 0.f;
+    uint32_t calls = 0;
+    if (ctx->ev_used) CK(cudaEventSynchronize(ctx->ev_pool[ctx->ev_used - 1]), "hough_profile_read synchronize");
+    for (size_t i = 0; i + 1 < ctx->ev_used; ++i) {
+        const int label = ctx->ev_label[i];
+        if (label < 0) { ++calls; continue; }                  // end of a call: the gap to the next call is nobody's
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ctx->ev_pool[i], ctx->ev_pool[i + 1]) == cudaSuccess) h_ms[label & 3] += ms;
+    }
+    if (ctx->ev_used) ++calls;
+    ctx->ev_used = 0;
+    if (h_calls) *h_calls = calls;
     return HOUGH_OK;
 }
 

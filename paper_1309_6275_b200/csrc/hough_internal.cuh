@@ -78,7 +78,11 @@ struct hough_ctx {
     uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
     hough_peak* d_hp_peaks; hough_track* d_hp_tracks; hough_jet* d_hp_jets;
     uint32_t* d_hp_npeaks; uint32_t* d_hp_njets; uint8_t* d_hp_flag;
-    std::vector<cudaEvent_t> ev_pool;         // hough_trigger_host stage timing: 4 per chunk, created on first use
+    // per-stage CUDA-event timing (hough_profile): marks recorded on the caller's stream around the launches
+    bool prof_on;
+    std::vector<cudaEvent_t> ev_pool;         // created on first use, reused, freed in hough_destroy
+    std::vector<int> ev_label;                // stage that STARTS at the mark (0 prep, 1 vote, 2 peaks, 3 jets), -1: end of a call
+    size_t ev_used;
     VotePlan vote;
     PeakPlan peak;
     cudaStream_t last_stream;

@@ -145,26 +145,44 @@ def test_displaced_truth_geometry_is_self_consistent():
 _SHARD_SCRIPT = r'''
 import os, sys
 import numpy as np
+import torch
 import torch.distributed as dist
 sys.path.insert(0, sys.argv[1])
 import bench
 rank = int(os.environ["RANK"]); world = int(os.environ["WORLD_SIZE"])
 dist.init_process_group("gloo", rank=rank, world_size=world)
+# strong-scaling helper: every event owned by exactly one rank
 lo, hi = bench.shard_range(37, rank, world)
 mine = np.zeros(37, np.int64); mine[lo:hi] = 1
-import torch
 t = torch.from_numpy(mine); dist.all_reduce(t)
-assert t.tolist() == [1] * 37, t.tolist()                       # every event owned by exactly one rank
+assert t.tolist() == [1] * 37, t.tolist()
+# the path run_ours takes (weak scaling): rank r owns events [r*E, (r+1)*E) of the stream, generates exactly those,
+# and the one exchange of the job gathers flag / n_peaks / n_jets of every rank.  The device calls are stubbed by
+# tensors whose values are a known function of the global event index.
+from paper_1309_6275_b200 import workloads as W
+E = 5
+w = W.scaled(W.config(5), n_events=E)
+first = bench.first_event_of_rank(E, rank)
+assert first == rank * E
+batch = W.generate(w, E, first_event=first)
+whole = W.generate(w, E * world)                                  # the stream every rank's slice comes from
+assert np.array_equal(batch.phi, whole.slice(first, first + E).phi)
+gidx = torch.arange(first, first + E)
+flag = (gidx % 3 == 0).to(torch.uint8); n_peaks = (gidx * 7 + 1).to(torch.int32); n_jets = (gidx + 2).to(torch.int32)
+gf, gp, gj = bench.gather_event_results(flag, n_peaks, n_jets, dist)
+allidx = torch.arange(E * world).reshape(world, E)
+assert gf.shape == (world, E) and torch.equal(gf, (allidx % 3 == 0).to(torch.uint8))
+assert torch.equal(gp, (allidx * 7 + 1).to(torch.int32)) and torch.equal(gj, (allidx + 2).to(torch.int32))
 ms = bench.max_over_ranks(10.0 + rank, dist)
 assert ms == 10.0 + world - 1
-tot = bench.sum_over_ranks(float(hi - lo), dist)
-assert tot == 37.0
+tot = bench.sum_over_ranks(float(E), dist)
+assert tot == float(E * world)
 dist.destroy_process_group()
 print("shard ok", rank, lo, hi)
 '''
 
 
-def test_event_sharding_world_size_2_gloo(tmp_path):
+def test_event_sharding_and_flag_gather_world_size_2_gloo(tmp_path):
     script = tmp_path / "shard.py"
     script.write_text(_SHARD_SCRIPT)
     env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29611")
@@ -173,3 +191,36 @@ def test_event_sharding_world_size_2_gloo(tmp_path):
                        capture_output=True, text=True, env=env, timeout=300)
     assert r.returncode == 0, r.stdout + r.stderr
     assert r.stdout.count("shard ok") == 2
+
+
+def test_bench_gpus_flag_is_checked_against_the_launch():
+    """--gpus N must match the number of ranks actually launched (round 1 silently ran one rank)."""
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "WORLD_SIZE=1" in (r.stdout + r.stderr)
+    import bench
+    assert bench.gather_event_results.__doc__ and bench.reexec_under_torchrun.__doc__
+
+
+def test_o2_instruction_count():
+    """bench.py's FP32 roofline term uses I_FP32 = FMA-pipe instructions (FADD / FMUL / FFMA) of the plain O-2 function
+    compiled for sm_100a.  Recount them from the SASS of csrc/o2_count.cu: fast path only (up to the
+    first EXIT; the slow path of the IEEE division sits behind it)."""
+    import bench
+    src = os.path.join(ROOT, "paper_1309_6275_b200", "csrc", "o2_count.cu")
+    cubin = str(os.path.join("/tmp", "hough_o2_count.cubin"))
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "--fmad=false", "-prec-div=true",
+                    "-ftz=false", "-cubin", src, "-o", cubin], check=True)
+    sass = subprocess.run(["cuobjdump", "-sass", cubin], capture_output=True, text=True, check=True).stdout
+    counts = {}
+    for body in sass.split("Function : ")[1:]:
+        name = body.split("\n")[0].strip()
+        fast = body.split("EXIT")[0]
+        ops = re.findall(r"^\s+/\*[0-9a-f]{4}\*/\s+(?:@!?U?P\d\s+)?([A-Z0-9_.]+)", fast, flags=re.M)
+        fma_pipe = [o for o in ops if o.split(".")[0] in ("FADD", "FMUL", "FFMA")]
+        other_fp = [o for o in ops if o.split(".")[0] in ("MUFU", "FCHK", "F2I", "FSETP")]
+        counts[name] = (len(fma_pipe), len(other_fp))
+    assert counts["o2_vote_3d"][0] == bench.I_FP32["3d"] == 17, counts
+    assert counts["o2_vote_2d"][0] == bench.I_FP32["2d"] == 11, counts
+    assert counts["o2_vote_3d"][1] == counts["o2_vote_2d"][1] == 5, counts        # MUFU.RCP, FCHK, F2I, 2 x FSETP
