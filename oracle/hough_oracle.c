@@ -333,3 +333,174 @@ uint32_t oracle_jets(const oracle_grid *g, const oracle_peak *peaks, uint32_t n_
     free(a); free(ipj); free(dsp); free(assigned);
     return J;
 }
+
+/* ================================================================================================ */
+/* O-6 / O-7: the paper's SECOND Hough transform -- tracks -> displaced vertices (PAPER.md:117,       */
+/* section 6: "the corresponding parameter space representation of these tracks is processed by a   */
+/* second application of the Hough transform ... to identify not straight lines but sinusoids which */
+/* contain a significant number of tracks, indicating that this is a location of a displaced jet";  */
+/* "the same peak finding algorithm is applied to the parameter space of this second Hough          */
+/* transform"; features at the interaction point are excluded "by setting a lower     */
+/* bound on the radius").  The paper gives no formula; readings R34-R39 fix it:           */
+/*   - vertex space = (phi_v, R_v) bins, phi_v periodic over [0, 2pi), R_v over [r_min, r_max) with  */
+/*     r_min the beam-pipe radius (the paper's lower bound); lin = iv * NR + ir (R_v fastest);       */
+/*   - a track (d0, phi0, kappa) (R1 convention) crosses the circle of radius r about the origin on  */
+/*     its outgoing branch at azimuth phi0 + asin(s), s = (kappa (r^2 + d0^2) - 2 d0) /              */
+/*     (2 r (1 - kappa d0)) (north_star's curvature formula solved for s; to first order             */
+/*     d0 = -r s = R_v sin(phi0 - phi_v): the sinusoid of the paper); one vote per (track, R_v bin)  */
+/*     at the bin centre radius, into the phi_v bin that holds the crossing azimuth;                 */
+/*   - no transcendental per vote: (cos, sin) of the crossing azimuth by rotating the track's        */
+/*     (cos phi0, sin phi0) by (sqrt(1 - s^2), s), and the phi_v bin by comparing that direction     */
+/*     with the bin-edge directions (cross products, binary search inside the quadrant); every step  */
+/*     below is one IEEE fp32 operation (+, -, *, /, sqrt are all correctly rounded);                */
+/*   - tracks compatible with the interaction point, |d0| <= d0_cut (the displaced-track cut of R20),  */
+/*     do not vote: a track through the origin crosses EVERY radius at nearly its own phi0, so prompt  */
+/*     tracks that merely share a phi0 bin would pile up at all radii; this is the paper's            */
+/*     interaction-point filter applied to the transform's input as well as to its radius axis;       */
+/*   - peaks: rule O-3 on the (phi_v, R_v) grid with the count threshold n_min; oracle_vertices      */
+/*     literally calls oracle_peaks with a "thermometer" mask of min(count, 16) bits, so that        */
+/*     popcount(mask) >= n_min <=> count >= n_min for n_min <= 16.                                   */
+/* Pins: tests/test_oracle_pins.py P14-P17.                                                          */
+/* ================================================================================================ */
+
+typedef struct {
+    uint32_t n_phi, n_r;              /* phi_v bins (multiple of 4), R_v bins (multiple of 8: the peak finder's axis rule) */
+    float r_min, r_max;               /* mm; r_min = beam pipe radius (interaction-point filter) */
+} oracle_vgrid;
+
+typedef struct { float r, phi; uint32_t n_tracks, lin; } oracle_vertex;
+
+static float vtx_r_centre(const oracle_vgrid *v, uint32_t ir)
+{
+    return (float)((double)v->r_min + ((double)ir + 0.5) * (((double)v->r_max - (double)v->r_min) / (double)v->n_r));
+}
+static double vtx_phi_edge(const oracle_vgrid *v, uint32_t k) { return (double)k * (2.0 * M_PI / (double)v->n_phi); }
+
+/* phi_v bin of the direction (x, y): quadrant from the signs, then the largest edge k of the quadrant with
+   cross(e_k, (x, y)) >= 0, by binary search; e_k = (cos, sin)(k * 2pi/n_phi) rounded once from double. */
+static uint32_t angle_bin(const oracle_vgrid *v, const float *ex, const float *ey, float x, float y)
+{
+    uint32_t q;                                   /* [0,pi/2): x>0,y>=0  [pi/2,pi): x<=0,y>0  [pi,3pi/2): x<0,y<=0  else */
+    if (x > 0.0f && y >= 0.0f) q = 0u;
+    else if (x <= 0.0f && y > 0.0f) q = 1u;
+    else if (x < 0.0f && y <= 0.0f) q = 2u;
+    else q = 3u;
+    uint32_t lo = q * (v->n_phi / 4u), hi = lo + v->n_phi / 4u - 1u;
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi + 1u) / 2u;
+        const float a = ex[mid] * y;
+        const float b = ey[mid] * x;
+        const float cr = a - b;
+        if (cr >= 0.0f) lo = mid; else hi = mid - 1u;
+    }
+    return lo;
+}
+
+/* exported for the pins */
+uint32_t oracle_angle_bin(const oracle_vgrid *v, float x, float y)
+{
+    float *ex = (float *)malloc(sizeof(float) * v->n_phi), *ey = (float *)malloc(sizeof(float) * v->n_phi);
+    for (uint32_t k = 0; k < v->n_phi; ++k) { ex[k] = (float)cos(vtx_phi_edge(v, k)); ey[k] = (float)sin(vtx_phi_edge(v, k)); }
+    const uint32_t b = angle_bin(v, ex, ey, x, y);
+    free(ex); free(ey);
+    return b;
+}
+
+/*
+ * O-6 vote: tracks given by fp32 parameters d0 [mm], (s0, c0) = (sin, cos) phi0, kappa [1/mm].
+ * count is the vertex plane [n_phi][n_r] (caller zeroes).  Returns the number of votes.
+ */
+int64_t oracle_vertex_vote(const oracle_vgrid *v, uint32_t n_tracks, const float *d0, const float *s0, const float *c0,
+                           const float *kappa, float d0_cut, uint16_t *count)
+{
+    float *ex = (float *)malloc(sizeof(float) * v->n_phi), *ey = (float *)malloc(sizeof(float) * v->n_phi);
+    for (uint32_t k = 0; k < v->n_phi; ++k) { ex[k] = (float)cos(vtx_phi_edge(v, k)); ey[k] = (float)sin(vtx_phi_edge(v, k)); }
+    int64_t votes = 0;
+    for (uint32_t j = 0; j < n_tracks; ++j) {
+        if (!(fabsf(d0[j]) > d0_cut)) continue;    /* prompt-compatible track: does not vote */
+        const float kd = kappa[j] * d0[j];
+        const float w = 1.0f - kd;                 /* 1 - kappa d0 */
+        const float d2 = d0[j] * d0[j];
+        const float two_d0 = 2.0f * d0[j];         /* exact */
+        for (uint32_t ir = 0; ir < v->n_r; ++ir) {
+            const float r = vtx_r_centre(v, ir);
+            const float r2 = r * r;
+            const float t1 = r2 + d2;
+            const float t2 = kappa[j] * t1;
+            const float num = t2 - two_d0;         /* kappa (r^2 + d0^2) - 2 d0 */
+            const float two_r = 2.0f * r;          /* exact */
+            const float den = two_r * w;           /* 2 r (1 - kappa d0) */
+            const float s = num / den;             /* sin of the crossing azimuth relative to phi0 */
+            if (!(fabsf(s) <= 1.0f)) continue;     /* the track does not reach radius r (NaN fails too) */
+            const float ss = s * s;
+            const float om = 1.0f - ss;
+            const float cd = sqrtf(om);            /* outgoing branch: cos >= 0 */
+            const float xa = c0[j] * cd;
+            const float xb = s0[j] * s;
+            const float x = xa - xb;               /* cos(phi0 + asin s) */
+            const float ya = s0[j] * cd;
+            const float yb = c0[j] * s;
+            const float y = ya + yb;               /* sin(phi0 + asin s) */
+            const uint32_t iv = angle_bin(v, ex, ey, x, y);
+            const size_t b = (size_t)iv * v->n_r + ir;
+            count[b] = (uint16_t)(count[b] + 1);
+            ++votes;
+        }
+    }
+    free(ex); free(ey);
+    return votes;
+}
+
+/*
+ * O-6 + O-7 for one event's stored peaks of the FIRST transform: bin-centre track parameters
+ * (d0c, phi0c tables of O-0; kappa_c = (float)(-kmax + (ik + 1/2) 2 kmax / NK) from double), vote, then the SAME
+ * peak finder (oracle_peaks, rule O-3: phi_v periodic, R_v clipped, ties to the lower lin) with threshold n_min
+ * (1..16) on the vertex plane.  Writes the first max_vertices vertices, returns the total; *flag = total > 0.
+ * count_out (may be NULL) receives the vertex plane [n_phi][n_r].
+ */
+uint32_t oracle_vertices(const oracle_grid *g, const oracle_vgrid *v, const oracle_peak *peaks, uint32_t n_stored,
+                         float d0_cut, uint32_t n_min, uint32_t max_vertices, oracle_vertex *out, uint8_t *flag,
+                         uint16_t *count_out)
+{
+    const size_t bins = (size_t)v->n_phi * v->n_r;
+    uint16_t *count = (uint16_t *)calloc(bins, sizeof(uint16_t));
+    uint16_t *mask = (uint16_t *)calloc(bins, sizeof(uint16_t));
+    float *d0 = (float *)malloc(sizeof(float) * (n_stored ? n_stored : 1));
+    float *s0 = (float *)malloc(sizeof(float) * (n_stored ? n_stored : 1));
+    float *c0 = (float *)malloc(sizeof(float) * (n_stored ? n_stored : 1));
+    float *kap = (float *)malloc(sizeof(float) * (n_stored ? n_stored : 1));
+    const double kmax = (double)g->kappa_max;
+    for (uint32_t j = 0; j < n_stored; ++j) {
+        const uint32_t lin = peaks[j].lin;
+        const uint32_t ik = lin % g->n_kappa;
+        const uint32_t ip = (lin / g->n_kappa) % g->n_phi0;
+        const uint32_t id = lin / g->n_kappa / g->n_phi0;
+        d0[j] = d0_centre(g, id);
+        s0[j] = (float)sin(phi0_centre(g, ip));
+        c0[j] = (float)cos(phi0_centre(g, ip));
+        kap[j] = (float)(-kmax + ((double)ik + 0.5) * (2.0 * kmax / (double)g->n_kappa));
+    }
+    oracle_vertex_vote(v, n_stored, d0, s0, c0, kap, d0_cut, count);
+    for (size_t b = 0; b < bins; ++b) {                       /* thermometer mask: popcount = min(count, 16) */
+        const uint32_t c = count[b] < 16 ? count[b] : 16;
+        mask[b] = (uint16_t)((1u << c) - 1u);
+    }
+    /* the same peak finder, on a 2D grid whose periodic axis is phi_v and whose clipped axis is R_v */
+    oracle_grid pg;
+    memset(&pg, 0, sizeof(pg));
+    pg.n_d0 = 1; pg.n_phi0 = v->n_phi; pg.n_kappa = v->n_r; pg.n_layers = 16;
+    oracle_peak *pk = (oracle_peak *)malloc(sizeof(oracle_peak) * (max_vertices ? max_vertices : 1));
+    const uint64_t total = oracle_peaks(&pg, count, mask, n_min, max_vertices, pk);
+    const uint64_t n_out = total < max_vertices ? total : max_vertices;
+    for (uint64_t i = 0; i < n_out; ++i) {
+        const uint32_t iv = pk[i].lin / v->n_r, ir = pk[i].lin % v->n_r;
+        out[i].r = vtx_r_centre(v, ir);
+        out[i].phi = (float)(((double)iv + 0.5) * (2.0 * M_PI / (double)v->n_phi));
+        out[i].n_tracks = pk[i].count;
+        out[i].lin = pk[i].lin;
+    }
+    *flag = total > 0 ? 1 : 0;
+    if (count_out) memcpy(count_out, count, bins * sizeof(uint16_t));
+    free(count); free(mask); free(d0); free(s0); free(c0); free(kap); free(pk);
+    return (uint32_t)total;
+}

@@ -28,6 +28,13 @@ JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced"
                       ("phi", "<f4"), ("sum_pt", "<f4")])
 
 
+VERTEX_DTYPE = np.dtype([("r", "<f4"), ("phi", "<f4"), ("n_tracks", "<u4"), ("lin", "<u4")])
+
+
+class _VGrid(C.Structure):
+    _fields_ = [("n_phi", C.c_uint32), ("n_r", C.c_uint32), ("r_min", C.c_float), ("r_max", C.c_float)]
+
+
 class _Grid(C.Structure):
     _fields_ = [("n_phi0", C.c_uint32), ("n_kappa", C.c_uint32), ("n_d0", C.c_uint32),
                 ("kappa_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float),
@@ -65,6 +72,13 @@ def _load():
         lib.oracle_jets.argtypes = [C.POINTER(_Grid), p, C.c_uint32, C.c_float, C.c_float, C.c_uint32,
                                     C.c_uint32, p, p, p]
         lib.oracle_jets.restype = C.c_uint32
+        lib.oracle_angle_bin.argtypes = [C.POINTER(_VGrid), C.c_float, C.c_float]
+        lib.oracle_angle_bin.restype = C.c_uint32
+        lib.oracle_vertex_vote.argtypes = [C.POINTER(_VGrid), C.c_uint32, p, p, p, p, C.c_float, p]
+        lib.oracle_vertex_vote.restype = C.c_int64
+        lib.oracle_vertices.argtypes = [C.POINTER(_Grid), C.POINTER(_VGrid), p, C.c_uint32, C.c_float, C.c_uint32,
+                                        C.c_uint32, p, p, p]
+        lib.oracle_vertices.restype = C.c_uint32
         _lib = lib
     return _lib
 
@@ -96,6 +110,50 @@ class Grid:
     @classmethod
     def from_workload(cls, w) -> "Grid":
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers)
+
+
+@dataclass(frozen=True)
+class VGrid:
+    """Vertex space of the second Hough transform: phi_v x R_v bins, R_v over [r_min, r_max) (r_min = beam pipe)."""
+    n_phi: int = 256
+    n_r: int = 128
+    r_min: float = 30.0
+    r_max: float = 430.0
+
+    def c(self) -> _VGrid:
+        return _VGrid(self.n_phi, self.n_r, self.r_min, self.r_max)
+
+    @property
+    def shape(self) -> Tuple[int, int]:
+        return (self.n_phi, self.n_r)
+
+
+def angle_bin(v: VGrid, x: float, y: float) -> int:
+    cv = v.c()
+    return int(_load().oracle_angle_bin(C.byref(cv), x, y))
+
+
+def vertex_vote(v: VGrid, d0, s0, c0, kappa, d0_cut: float = -1.0):
+    """O-6 for tracks given by fp32 parameters: (count uint16 [n_phi, n_r], votes); tracks with |d0| <= d0_cut do not
+    vote (the default -1 lets every track vote)."""
+    d0 = np.ascontiguousarray(d0, np.float32); s0 = np.ascontiguousarray(s0, np.float32)
+    c0 = np.ascontiguousarray(c0, np.float32); kappa = np.ascontiguousarray(kappa, np.float32)
+    count = np.zeros(v.shape, np.uint16)
+    cv = v.c()
+    n = _load().oracle_vertex_vote(C.byref(cv), d0.size, _ptr(d0), _ptr(s0), _ptr(c0), _ptr(kappa), d0_cut, _ptr(count))
+    return count, int(n)
+
+
+def vertices(g: Grid, v: VGrid, pk: np.ndarray, d0_cut_mm: float, n_min: int, max_vertices: int):
+    """O-6 + O-7 for ONE event's stored peaks: (stored vertices, total, flag, vertex plane)."""
+    pk = np.ascontiguousarray(pk, PEAK_DTYPE)
+    out = np.zeros(max_vertices, VERTEX_DTYPE)
+    flag = np.zeros(1, np.uint8)
+    count = np.zeros(v.shape, np.uint16)
+    cg, cv = g.c(), v.c()
+    n = int(_load().oracle_vertices(C.byref(cg), C.byref(cv), _ptr(pk), pk.size, d0_cut_mm, n_min, max_vertices,
+                                    _ptr(out), _ptr(flag), _ptr(count)))
+    return out[:min(n, max_vertices)].copy(), n, int(flag[0]), count
 
 
 def tables(g: Grid):
