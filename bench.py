@@ -46,6 +46,7 @@ I_FP32 = {"3d": 17.0, "2d": 11.0}
 # column (SURVEY.md 8(d) counts them "per (hit, ip)"): a stricter denominator, reported next to the contract's
 I_FP32_SHARED = {"3d": 12.0, "2d": 11.0}
 SM_COUNT, FP32_LANES = 148, 128
+STAGES = ("prep", "vote", "peaks", "jets", "vertices")
 SMEM_RED_PER_CLK = 32                                         # conflict-free 32-bit shared reductions per clock and SM
 
 
@@ -277,7 +278,7 @@ def run_reference(args):
 class DeviceRun:
     """One workload resident on the device: context, uploaded hits, output tensors, and the step function."""
 
-    def __init__(self, w, batch, chunk: int, path: str):
+    def __init__(self, w, batch, chunk: int, path: str, vertices: bool = True):
         import torch
         from paper_1309_6275_b200 import binding as B
         self.torch, self.B, self.w, self.batch, self.path = torch, B, w, batch, path
@@ -286,7 +287,9 @@ class DeviceRun:
         self.offs = batch.hit_offsets.astype(np.int64)
         self.n_chunks = (self.E + self.chunk - 1) // self.chunk
         hits_per_chunk = max(int(self.offs[min(c + self.chunk, self.E)] - self.offs[c]) for c in range(0, self.E, self.chunk))
-        self.h = B.Hough.for_workload(w, max_events=self.chunk, max_hits=max(1, hits_per_chunk))
+        self.vertices = vertices and w.n_d0 > 1                  # the second Hough transform needs displaced tracks
+        self.h = B.Hough.for_workload(w, max_events=self.chunk, max_hits=max(1, hits_per_chunk),
+                                      vgrid=w.vgrid if self.vertices else None, max_vertices=w.max_vertices)
         self.off, self.r, self.phi, self.layer = B.upload_batch(batch)
         self.out = self.h.alloc_outputs(self.E)
         self.count = self.mask = None
@@ -308,9 +311,12 @@ class DeviceRun:
                 h.hough_peaks(ne, self.count, self.mask, w.l_min, out["peaks"][e0:], out["n_peaks"][e0:], st)
             h.hough_jets(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.cone_rad, w.d0_cut_mm, w.n_displaced_min,
                          out["tracks"][e0:], out["jets"][e0:], out["n_jets"][e0:], out["flag"][e0:], st)
+            if self.vertices:
+                h.hough_vertices(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.d0_cut_mm, w.vtx_n_min, out["vertices"][e0:],
+                                 out["n_vertices"][e0:], out["vtx_flag"][e0:], None, st)
 
     def timed(self, steps: int, warmup: int, dist=None, after_step=None):
-        """(ms total, stage ms {prep, vote, peaks, jets}, launches) for `steps` steps after `warmup` untimed ones."""
+        """(ms total, stage ms {prep, vote, peaks, jets, vertices}, launches) for `steps` steps after `warmup` untimed ones."""
         torch = self.torch
         for _ in range(warmup):
             self.step()
@@ -414,7 +420,7 @@ def measure_config(name: str, hbm_gbs, sm_max_mhz, peak_src, steps: int = 3):
         ms, stage, launches = run.timed(reps, 20 if single else 2)
         n_launch = reps * run.n_chunks
         d = {"ms_per_step": ms / reps, "events_per_sec": w.n_events * reps / (ms * 1e-3),
-             "stage_ms_per_step": {k: v / reps for k, v in zip(("prep", "vote", "peaks", "jets"), stage)},
+             "stage_ms_per_step": {k: v / reps for k, v in zip(STAGES, stage)},
              "launches_per_step": launches // reps}
         if single:
             d["latency_us"] = 1e3 * ms / reps
@@ -462,7 +468,7 @@ def run_ours(args):
 
     votes_per_step = count_votes(w, batch)
 
-    run = DeviceRun(w, batch, chunk, args.path)
+    run = DeviceRun(w, batch, chunk, args.path, vertices=not args.no_vertices)
     gathered = {}
 
     def exchange():
@@ -478,6 +484,11 @@ def run_ours(args):
     clocks = sampler.stop(wall0 + 0.0, wall1)
     status = run.h.hough_status()
     n_flag = int(run.out["flag"].sum().item())
+    n_vflag = int(run.out["vtx_flag"].sum().item()) if run.vertices else None
+    n_vtx_total = int(run.out["n_vertices"].to(torch.int64).sum().item()) if run.vertices else None
+    n_both = int((run.out["flag"].bool() & run.out["vtx_flag"].bool()).sum().item()) if run.vertices else None
+    vflags_dev = run.out["vtx_flag"].cpu().numpy().copy()
+    with_vtx = run.vertices
     n_peaks_total = int(run.out["n_peaks"].to(torch.int64).sum().item())
     flags_dev = run.out["flag"].cpu().numpy().copy()
     npk_dev = run.out["n_peaks"].cpu().numpy().copy()
@@ -505,7 +516,7 @@ def run_ours(args):
         p_ms, p_stage, p_launches = prun.timed(p_steps, 1)
         pl = p_steps * prun.n_chunks
         planes = {"events": n_ev, "ms_per_step": p_ms / p_steps, "events_per_sec": n_ev * p_steps / (p_ms * 1e-3),
-                  "stage_ms_per_step": {k: v / p_steps for k, v in zip(("prep", "vote", "peaks", "jets"), p_stage)},
+                  "stage_ms_per_step": {k: v / p_steps for k, v in zip(STAGES, p_stage)},
                   "roofline_vote": vote_roofline(mode, votes_sub * p_steps, bins * n_ev * p_steps, p_stage[1], pl, hbm_gbs,
                                                  sm_max_mhz, peak_src, "vote_kernel"),
                   "roofline_stencil": stencil_roofline(bins * n_ev * p_steps, p_stage[2], pl, hbm_gbs)}
@@ -516,7 +527,8 @@ def run_ours(args):
         torch.cuda.empty_cache()
 
     # ---- e2e: the same batch through hough_trigger_host with pinned host buffers ----
-    h2 = B.Hough.for_workload(w, max_events=E, max_hits=H, host_chunk_events=chunk)
+    h2 = B.Hough.for_workload(w, max_events=E, max_hits=H, host_chunk_events=chunk,
+                              vgrid=w.vgrid if with_vtx else None, max_vertices=w.max_vertices)
     pin = lambda a: torch.from_numpy(a).pin_memory()
     h_off, h_r, h_phi, h_layer = pin(batch.hit_offsets.view(np.int32)), pin(batch.r), pin(batch.phi), pin(batch.layer)
     h_np = torch.zeros(E, dtype=torch.int32).pin_memory(); h_nj = torch.zeros(E, dtype=torch.int32).pin_memory()
@@ -524,8 +536,15 @@ def run_ours(args):
     h_jets = torch.zeros((E, w.max_jets, 20), dtype=torch.uint8).pin_memory()
     stream = torch.cuda.current_stream()
     e2e_steps = max(1, min(args.steps, 3))
-    call = lambda: h2.hough_trigger_host(E, h_off, H, h_r, h_phi, h_layer, w.l_min, w.cone_rad, w.d0_cut_mm,
-                                         w.n_displaced_min, h_np, h_nj, h_fl, None, h_jets, None, stream)
+    h_nv = torch.zeros(E, dtype=torch.int32).pin_memory(); h_vf = torch.zeros(E, dtype=torch.uint8).pin_memory()
+    h_vtx = torch.zeros((E, w.max_vertices, 16), dtype=torch.uint8).pin_memory()
+    if with_vtx:
+        call = lambda: h2.hough_trigger_host_vtx(E, h_off, H, h_r, h_phi, h_layer, w.l_min, w.cone_rad, w.d0_cut_mm,
+                                                 w.n_displaced_min, w.vtx_n_min, h_np, h_nj, h_fl, None, h_jets, h_nv,
+                                                 h_vf, h_vtx, None, stream)
+    else:
+        call = lambda: h2.hough_trigger_host(E, h_off, H, h_r, h_phi, h_layer, w.l_min, w.cone_rad, w.d0_cut_mm,
+                                             w.n_displaced_min, h_np, h_nj, h_fl, None, h_jets, None, stream)
     call()
     torch.cuda.synchronize()
     if dist: dist.barrier()
@@ -537,7 +556,8 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_e2e = max_over_ranks(a.elapsed_time(b), dist)
     e2e_value = sum_over_ranks(float(E * e2e_steps), dist) / (ms_e2e * 1e-3)
-    e2e_ok = bool(np.array_equal(h_fl.numpy(), flags_dev) and np.array_equal(h_np.numpy(), npk_dev))
+    e2e_ok = bool(np.array_equal(h_fl.numpy(), flags_dev) and np.array_equal(h_np.numpy(), npk_dev) and
+                  (not with_vtx or np.array_equal(h_vf.numpy(), vflags_dev)))
     h2_launches = h2.hough_launch_count()
     h2.close()
     torch.cuda.empty_cache()
@@ -574,11 +594,15 @@ def run_ours(args):
                    "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min, "cone_rad": w.cone_rad, "l2": l2_note},
         "votes_per_sec": votes_timed * world / (ms_max * 1e-3) if world == 1 else None,
         "votes_per_step": votes_per_step,
-        "stage_ms_per_step": {k: v / args.steps for k, v in zip(("prep", "vote", "peaks", "jets"), stage)},
+        "stage_ms_per_step": {k: v / args.steps for k, v in zip(STAGES, stage)},
         "events_flagged": n_flag, "events_flagged_all_ranks": job_flags, "peaks_total": n_peaks_total,
+        "second_transform": ({"vertex_grid": list(w.vgrid), "n_min": w.vtx_n_min, "d0_cut_mm": w.d0_cut_mm,
+                              "events_flagged_vertex": n_vflag, "vertices_total": n_vtx_total,
+                              "events_flagged_by_both": n_both} if with_vtx else None),
         "status_bits": status, "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": int(H * 9 + (E + 1) * 4),
-                "d2h_bytes_per_step": int(E * 9 + E * w.max_jets * 20), "steps": e2e_steps,
+                "d2h_bytes_per_step": int(E * 9 + E * w.max_jets * 20 + (E * 5 + E * w.max_vertices * 16 if with_vtx else 0)),
+                "steps": e2e_steps,
                 "matches_device_path": e2e_ok},
         "gpu_launches": int(launches), "gpu_launches_e2e": int(h2_launches),
         "roofline": roofline,
@@ -607,6 +631,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--no-planes-leg", action="store_true")
+    ap.add_argument("--no-vertices", action="store_true", help="leave the second Hough transform out of the step")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -49,11 +49,18 @@ typedef struct {
                                       and hough_vote_peaks accepts at most host_chunk_events events per call        */
     uint32_t max_candidates_per_event; /* fused path: capacity of the per-event peak-candidate buffer (16 B each);
                                       0 = default max(4 * max_peaks_per_event, 4096)                                  */
+    /* vertex space of the second Hough transform (hough_vertices); n_vtx_phi == 0 disables it */
+    uint32_t n_vtx_phi;            /* phi_v bins over [0, 2pi), periodic; multiple of 4, >= 8                         */
+    uint32_t n_vtx_r;              /* R_v bins over [vtx_r_min, vtx_r_max), half-open; multiple of 8, >= 8;
+                                      n_vtx_phi * n_vtx_r * 2 bytes must fit in shared memory (<= 200 KB)            */
+    float    vtx_r_min, vtx_r_max; /* mm; vtx_r_min = radius inside which vertices are dropped (beam pipe, 30 mm)     */
+    uint32_t max_vertices_per_event;
 } hough_config;
 
 typedef struct { uint32_t lin; uint16_t count; uint16_t mask; } hough_peak;                     /*  8 B */
 typedef struct { float pt, phi0, d0; int32_t q; int32_t jet; } hough_track;                     /* 20 B */
 typedef struct { uint32_t seed_track, n_tracks, n_displaced; float phi, sum_pt; } hough_jet;    /* 20 B */
+typedef struct { float r, phi; uint32_t n_tracks; uint32_t lin; } hough_vertex;                 /* 16 B */
 
 enum {
     HOUGH_OK = 0,
@@ -158,6 +165,30 @@ int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, con
                hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag, void* stream);
 
 /*
+ * The paper's SECOND Hough transform: tracks -> displaced vertices (section 6: "the corresponding
+ * parameter space representation of these tracks is processed by a second application of the Hough transform ...
+ * to identify not straight lines but sinusoids which contain a significant number of tracks ... the same peak
+ * finding algorithm is applied to the parameter space of this second Hough transform"; the tracks from
+ * the interaction point are excluded "by setting a lower bound on the radius"; cost proportional to
+ * the number of tracks).  DESIGN.md O-6 / O-7.
+ * For the T = min(n_peaks, max_peaks) stored peaks of each event (bin-centre track parameters d0c, phi0c, kappa_c):
+ * every track with |d0c| > d0_cut_mm votes, for each R_v bin centre r it reaches, into the phi_v bin of the azimuth
+ * phi0 + asin(s), s = (kappa (r^2 + d0^2) - 2 d0) / (2 r (1 - kappa d0)), at which its outgoing branch crosses
+ * radius r (to first order d0 = R_v sin(phi0 - phi_v): the sinusoid of the paper), in IEEE fp32 without a
+ * transcendental per vote.  Vertices = bins of the (phi_v, R_v) plane with count >= n_min that are strict local
+ * maxima of (count, -lin) over the 3x3 neighbourhood (phi_v periodic, R_v clipped), lin = iv * NR + ir, in
+ * ascending lin; r / phi are bin centres, n_tracks the count.
+ *   d_vertices   [n_events][max_vertices_per_event]; d_n_vertices [n_events] u32 TRUE total; d_flag [n_events] u8
+ *   = 1 iff the event has a vertex;  d_vertex_plane: optional (may be null) [n_events][n_vtx_phi][n_vtx_r] u16,
+ *   receives the vote counts (tests).
+ * n_min in [1, 65535] (the oracle's peak-finder reuse covers 1..16).  HOUGH_EINVAL if the context was created
+ * without a vertex grid.
+ */
+int hough_vertices(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                   float d0_cut_mm, uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices, uint8_t* d_flag,
+                   uint16_t* d_vertex_plane, void* stream);
+
+/*
  * End-to-end trigger on HOST buffers (the call bench.py's e2e leg times): copies the hits to the device,
  * runs the fused vote -> peaks path and the jets in launches of cfg.host_chunk_events events, and copies
  * n_peaks / n_jets / flag (and, if non-null, peaks and jets) back.  Events that overflowed the candidate buffer
@@ -175,6 +206,20 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
                        hough_jet* h_jets /* [n_events][max_jets] or null */,
                        float* ms_stage /* [3] or null */, void* stream);
 
+/*
+ * The same with the second Hough transform run after the jets (context created with a vertex grid):
+ * h_n_vertices [n_events] u32, h_vtx_flag [n_events] u8, h_vertices [n_events][max_vertices] or null.
+ * ms_stage, if not null, has FOUR entries: {vote, peaks, jets, vertices}.
+ */
+int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
+                           const float* h_r, const float* h_phi, const uint8_t* h_layer,
+                           uint32_t l_min, float cone_rad, float d0_cut_mm, uint32_t n_displaced_min,
+                           uint32_t vtx_n_min,
+                           uint32_t* h_n_peaks, uint32_t* h_n_jets, uint8_t* h_flag,
+                           hough_peak* h_peaks, hough_jet* h_jets,
+                           uint32_t* h_n_vertices, uint8_t* h_vtx_flag, hough_vertex* h_vertices,
+                           float* ms_stage /* [4] or null */, void* stream);
+
 /* Synchronises the stream of the last call on ctx and returns (and keeps) the sticky status bits.  HOST out. */
 int hough_status(hough_ctx* ctx, uint32_t* host_status_bits);
 
@@ -182,11 +227,11 @@ int hough_status(hough_ctx* ctx, uint32_t* host_status_bits);
  * Per-stage device timing with CUDA events on the caller's stream (what bench.py's roofline uses).  While enabled,
  * every call on ctx records an event before each stage and one at its end.  hough_profile_read waits for the last
  * recorded event and returns the milliseconds accumulated since the previous read in
- * h_ms[0..3] = {hit preparation, vote kernel, peak kernels (stencil + compaction, or recount + ordering), jets}
- * and the number of calls seen.  HOST out.  Costs one event record (a few microseconds) per stage while enabled.
+ * h_ms[0..4] = {hit preparation, vote kernel, peak kernels (stencil + compaction, or recount + ordering), jets,
+ * vertices} and the number of calls seen.  HOST out.  Costs one event record (a few microseconds) per stage while enabled.
  */
 int hough_profile(hough_ctx* ctx, int enable);
-int hough_profile_read(hough_ctx* ctx, float* h_ms /* [4] */, uint32_t* h_calls /* may be null */);
+int hough_profile_read(hough_ctx* ctx, float* h_ms /* [5] */, uint32_t* h_calls /* may be null */);
 
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches).  HOST out. */
 int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);

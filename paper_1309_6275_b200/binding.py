@@ -19,12 +19,13 @@ PEAK_DTYPE = np.dtype([("lin", "<u4"), ("count", "<u2"), ("mask", "<u2")])
 TRACK_DTYPE = np.dtype([("pt", "<f4"), ("phi0", "<f4"), ("d0", "<f4"), ("q", "<i4"), ("jet", "<i4")])
 JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced", "<u4"),
                       ("phi", "<f4"), ("sum_pt", "<f4")])
+VERTEX_DTYPE = np.dtype([("r", "<f4"), ("phi", "<f4"), ("n_tracks", "<u4"), ("lin", "<u4")])
 
 ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING, ST_CANDIDATE_OVERFLOW = 1, 2, 4, 8
 ST_ERRORS = ST_EVENT_TOO_LARGE | ST_BAD_OFFSETS            # the bits that mean "results undefined"
 N_PEAKS_OVERFLOW = 0xFFFFFFFF
 EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_vote_peaks",
-           "hough_jets",
+           "hough_jets", "hough_vertices", "hough_trigger_host_vtx",
            "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
            "hough_debug_prepared_hits", "hough_debug_div_check", "hough_profile", "hough_profile_read"]
 
@@ -34,7 +35,9 @@ class HoughConfig(C.Structure):
                 ("kappa_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float), ("b_tesla", C.c_float),
                 ("n_layers", C.c_uint32), ("max_events", C.c_uint32), ("max_hits", C.c_uint64),
                 ("max_peaks_per_event", C.c_uint32), ("max_jets_per_event", C.c_uint32),
-                ("host_chunk_events", C.c_uint32), ("max_candidates_per_event", C.c_uint32)]
+                ("host_chunk_events", C.c_uint32), ("max_candidates_per_event", C.c_uint32),
+                ("n_vtx_phi", C.c_uint32), ("n_vtx_r", C.c_uint32), ("vtx_r_min", C.c_float), ("vtx_r_max", C.c_float),
+                ("max_vertices_per_event", C.c_uint32)]
 
 
 class HoughError(RuntimeError):
@@ -65,6 +68,8 @@ def load_library() -> C.CDLL:
         lib.hough_vote_peaks.argtypes = [p, u32, p, u64, p, p, p, u32, p, p, p]
         lib.hough_jets.argtypes = [p, u32, p, p, f32, f32, u32, p, p, p, p, p]
         lib.hough_trigger_host.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, p, p, p, p, p, p, p]
+        lib.hough_trigger_host_vtx.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, u32, p, p, p, p, p, p, p, p, p, p]
+        lib.hough_vertices.argtypes = [p, u32, p, p, f32, u32, p, p, p, p, p]
         lib.hough_status.argtypes = [p, C.POINTER(u32)]
         lib.hough_launch_count.argtypes = [p, C.POINTER(u64)]
         lib.hough_microbench.argtypes = [C.c_int, C.c_size_t, C.POINTER(C.c_double)]
@@ -121,18 +126,22 @@ class Hough:
     def __init__(self, n_phi0: int, n_kappa: int, n_d0: int = 1, kappa_max: float = 0.3e-3 * 3.8,
                  d0_min: float = 0.0, d0_max: float = 0.0, b_tesla: float = 3.8, n_layers: int = 8,
                  max_events: int = 1, max_hits: int = 1 << 16, max_peaks_per_event: int = 4096,
-                 max_jets_per_event: int = 256, host_chunk_events: int = 0, max_candidates_per_event: int = 0):
+                 max_jets_per_event: int = 256, host_chunk_events: int = 0, max_candidates_per_event: int = 0,
+                 n_vtx_phi: int = 0, n_vtx_r: int = 0, vtx_r_min: float = 30.0, vtx_r_max: float = 430.0,
+                 max_vertices_per_event: int = 64):
         self.lib = load_library()
         self.cfg = HoughConfig(n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, n_layers, max_events,
                                max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events,
-                               max_candidates_per_event)
+                               max_candidates_per_event, n_vtx_phi, n_vtx_r, vtx_r_min, vtx_r_max,
+                               max_vertices_per_event)
         self._ctx = C.c_void_p()
         _check(self.lib.hough_create(C.byref(self.cfg), C.byref(self._ctx)), "hough_create")
 
     @classmethod
     def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
                      host_chunk_events: int = 0, max_peaks: Optional[int] = None,
-                     max_candidates: int = 0) -> "Hough":
+                     max_candidates: int = 0, vgrid=None, max_vertices: int = 64) -> "Hough":
+        """vgrid: None, or (n_vtx_phi, n_vtx_r, r_min, r_max) for the second Hough transform (hough_vertices)."""
         ne = w.n_events if max_events is None else max_events
         if max_hits is None:
             raise ValueError("for_workload: pass max_hits (the hit count of the largest batch per call); the context "
@@ -140,7 +149,7 @@ class Hough:
         mh = max_hits
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
                    min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
-                   host_chunk_events, max_candidates)
+                   host_chunk_events, max_candidates, *((0, 0, 30.0, 430.0) if vgrid is None else vgrid), max_vertices)
 
     # -- lifetime ---------------------------------------------------------------------------------
     def close(self):
@@ -179,7 +188,11 @@ class Hough:
             tracks=torch.zeros((n_events, mp, TRACK_DTYPE.itemsize), dtype=torch.uint8, device=dev),
             jets=torch.zeros((n_events, mj, JET_DTYPE.itemsize), dtype=torch.uint8, device=dev),
             n_jets=torch.zeros(n_events, dtype=torch.int32, device=dev),
-            flag=torch.zeros(n_events, dtype=torch.uint8, device=dev))
+            flag=torch.zeros(n_events, dtype=torch.uint8, device=dev),
+            vertices=torch.zeros((n_events, max(1, self.cfg.max_vertices_per_event), VERTEX_DTYPE.itemsize),
+                                 dtype=torch.uint8, device=dev),
+            n_vertices=torch.zeros(n_events, dtype=torch.int32, device=dev),
+            vtx_flag=torch.zeros(n_events, dtype=torch.uint8, device=dev))
 
     # -- the hot path (device pointers + caller stream) -------------------------------------------
     def hough_vote(self, n_events, d_hit_offsets, n_hits_total, d_r, d_phi, d_layer, d_count, d_mask, stream=None):
@@ -201,6 +214,27 @@ class Hough:
         _check(self.lib.hough_jets(self._ctx, n_events, _dptr(d_peaks), _dptr(d_n_peaks), cone_rad, d0_cut_mm,
                                    n_displaced_min, _dptr(d_tracks), _dptr(d_jets), _dptr(d_n_jets), _dptr(d_flag),
                                    _stream_ptr(stream)), "hough_jets")
+
+    def hough_vertices(self, n_events, d_peaks, d_n_peaks, d0_cut_mm, n_min, d_vertices, d_n_vertices, d_flag,
+                       d_vertex_plane=None, stream=None):
+        plane = C.c_void_p(0) if d_vertex_plane is None else _dptr(d_vertex_plane)
+        _check(self.lib.hough_vertices(self._ctx, n_events, _dptr(d_peaks), _dptr(d_n_peaks), d0_cut_mm, n_min,
+                                       _dptr(d_vertices), _dptr(d_n_vertices), _dptr(d_flag), plane,
+                                       _stream_ptr(stream)), "hough_vertices")
+
+    def hough_trigger_host_vtx(self, n_events, h_hit_offsets, n_hits_total, h_r, h_phi, h_layer, l_min, cone_rad,
+                               d0_cut_mm, n_displaced_min, vtx_n_min, h_n_peaks, h_n_jets, h_flag, h_peaks, h_jets,
+                               h_n_vertices, h_vtx_flag, h_vertices=None, ms_stage=None, stream=None):
+        """hough_trigger_host + the second Hough transform; HOST tensors / arrays in and out."""
+        def hp(x):
+            if x is None:
+                return C.c_void_p(0)
+            return C.c_void_p(x.ctypes.data) if isinstance(x, np.ndarray) else C.c_void_p(x.data_ptr())
+        _check(self.lib.hough_trigger_host_vtx(self._ctx, n_events, hp(h_hit_offsets), n_hits_total, hp(h_r), hp(h_phi),
+                                               hp(h_layer), l_min, cone_rad, d0_cut_mm, n_displaced_min, vtx_n_min,
+                                               hp(h_n_peaks), hp(h_n_jets), hp(h_flag), hp(h_peaks), hp(h_jets),
+                                               hp(h_n_vertices), hp(h_vtx_flag), hp(h_vertices), hp(ms_stage),
+                                               _stream_ptr(stream)), "hough_trigger_host_vtx")
 
     def hough_trigger_host(self, n_events, h_hit_offsets, n_hits_total, h_r, h_phi, h_layer, l_min, cone_rad,
                            d0_cut_mm, n_displaced_min, h_n_peaks, h_n_jets, h_flag, h_peaks=None, h_jets=None,
@@ -232,8 +266,8 @@ class Hough:
         _check(self.lib.hough_profile(self._ctx, 1 if enable else 0), "hough_profile")
 
     def hough_profile_read(self):
-        """(ms per stage {prep, vote, peaks, jets} since the last read, number of calls)."""
-        ms = (C.c_float * 4)(); n = C.c_uint32(0)
+        """(ms per stage {prep, vote, peaks, jets, vertices} since the last read, number of calls)."""
+        ms = (C.c_float * 5)(); n = C.c_uint32(0)
         _check(self.lib.hough_profile_read(self._ctx, ms, C.byref(n)), "hough_profile_read")
         return [float(x) for x in ms], int(n.value)
 

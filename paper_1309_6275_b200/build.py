@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhough_b200.so")
-SOURCES = ["api.cu", "vote.cu", "peaks.cu", "jets.cu", "microbench.cu"]
+SOURCES = ["api.cu", "vote.cu", "peaks.cu", "jets.cu", "vertices.cu", "microbench.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "--fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
@@ -27,7 +27,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "hough.h")]
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != "o2_count.cu"] + [os.path.join(ROOT, "include", "hough.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -40,6 +40,8 @@ void free_all(hough_ctx* c)
     cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_cand); cudaFree(c->d_cand_n); cudaFree(c->d_sortkeys);
+    cudaFree(c->d_kc); cudaFree(c->d_vex); cudaFree(c->d_vey); cudaFree(c->d_vrc);
+    cudaFree(c->d_hp_vertices); cudaFree(c->d_hp_nvtx); cudaFree(c->d_hp_vflag);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
     cudaFree(c->d_hp_phi); cudaFree(c->d_hp_layer); cudaFree(c->d_hp_peaks); cudaFree(c->d_hp_tracks);
     cudaFree(c->d_hp_jets); cudaFree(c->d_hp_npeaks); cudaFree(c->d_hp_njets); cudaFree(c->d_hp_flag);
@@ -78,6 +80,12 @@ bool config_ok(const hough_config* g)
     if (g->max_peaks_per_event < 1 || g->max_jets_per_event < 1) return false;
     if (g->host_chunk_events > g->max_events) return false;
     if (g->max_candidates_per_event > (1u << 24)) return false;
+    if (g->n_vtx_phi != 0) {                                   // vertex grid of the second transform
+        if (g->n_vtx_phi < 8 || g->n_vtx_phi % 4 != 0 || g->n_vtx_r < 8 || g->n_vtx_r % 8 != 0) return false;
+        if ((uint64_t)g->n_vtx_phi * g->n_vtx_r * 2 > 200u * 1024u) return false;
+        if (!(g->vtx_r_min > 0.f) || !(g->vtx_r_max > g->vtx_r_min) || !isfinite(g->vtx_r_max)) return false;
+        if (g->max_vertices_per_event < 1) return false;
+    }
     return true;
 }
 
@@ -133,6 +141,20 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         volatile float dd = d * d;                    // one fp32 multiply, kept out of any contraction
         d0c[id] = d; two_d0[id] = 2.0f * d; d0sq[id] = dd;
     }
+    // O-6 tables: kappa bin centres, phi_v edge directions, R_v bin centres (double, rounded once)
+    std::vector<float> kc(NK), vex, vey, vrc;
+    for (uint32_t ik = 0; ik < NK; ++ik)
+        kc[ik] = (float)(-(double)cfg->kappa_max + ((double)ik + 0.5) * (2.0 * (double)cfg->kappa_max / (double)NK));
+    if (cfg->n_vtx_phi) {
+        vex.resize(cfg->n_vtx_phi); vey.resize(cfg->n_vtx_phi); vrc.resize(cfg->n_vtx_r);
+        for (uint32_t k = 0; k < cfg->n_vtx_phi; ++k) {
+            const double a = (double)k * (2.0 * pi / (double)cfg->n_vtx_phi);
+            vex[k] = (float)cos(a); vey[k] = (float)sin(a);
+        }
+        for (uint32_t ir = 0; ir < cfg->n_vtx_r; ++ir)
+            vrc[ir] = (float)((double)cfg->vtx_r_min +
+                              ((double)ir + 0.5) * (((double)cfg->vtx_r_max - (double)cfg->vtx_r_min) / (double)cfg->n_vtx_r));
+    }
     // the branch-free exact division of the vote kernel is only used inside this range (vote.cu, div_rn_tame)
     c->tame_tables = cfg->kappa_max >= 9.094947e-13f && cfg->kappa_max <= 1.0995116e12f;      // [2^-40, 2^40]
     for (uint32_t id = 0; id < ND; ++id) {
@@ -148,6 +170,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     auto A = [&](cudaError_t e2) { if (err == cudaSuccess) err = e2; };
     A(dev_alloc(&c->d_c0, NP)); A(dev_alloc(&c->d_s0, NP));
     A(dev_alloc(&c->d_d0c, ND)); A(dev_alloc(&c->d_two_d0, ND)); A(dev_alloc(&c->d_d0sq, ND));
+    A(dev_alloc(&c->d_kc, NK));
+    A(dev_alloc(&c->d_vex, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vey, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vrc, cfg->n_vtx_r));
     A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_rec_u, cfg->max_hits)); A(dev_alloc(&c->d_key, cfg->max_hits));
     A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
     A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
@@ -180,6 +204,10 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         A(dev_alloc(&c->d_hp_tracks, E * cfg->max_peaks_per_event));
         A(dev_alloc(&c->d_hp_jets, E * cfg->max_jets_per_event));
         A(dev_alloc(&c->d_hp_npeaks, E)); A(dev_alloc(&c->d_hp_njets, E)); A(dev_alloc(&c->d_hp_flag, E));
+        if (cfg->n_vtx_phi) {
+            A(dev_alloc(&c->d_hp_vertices, E * cfg->max_vertices_per_event));
+            A(dev_alloc(&c->d_hp_nvtx, E)); A(dev_alloc(&c->d_hp_vflag, E));
+        }
     }
     if (err != cudaSuccess) {
         cuda_fail(err, "hough_create allocation");
@@ -195,6 +223,12 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemcpy(c->d_two_d0, two_d0.data(), ND * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_d0sq, d0sq.data(), ND * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_kc, kc.data(), NK * 4, cudaMemcpyHostToDevice));
+    if (cfg->n_vtx_phi) {
+        A(cudaMemcpy(c->d_vex, vex.data(), vex.size() * 4, cudaMemcpyHostToDevice));
+        A(cudaMemcpy(c->d_vey, vey.data(), vey.size() * 4, cudaMemcpyHostToDevice));
+        A(cudaMemcpy(c->d_vrc, vrc.data(), vrc.size() * 4, cudaMemcpyHostToDevice));
+    }
     A(cudaMemset(c->d_status, 0, 8));
     A(cudaMemset(c->d_tilectr, 0, 8));
     A(cudaMemset(c->d_cand_n, 0, (size_t)c->fused_events * 4));
@@ -296,10 +330,28 @@ int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, con
     return HOUGH_OK;
 }
 
-int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
-                       const float* h_r, const float* h_phi, const uint8_t* h_layer, uint32_t l_min, float cone_rad,
-                       float d0_cut_mm, uint32_t n_displaced_min, uint32_t* h_n_peaks, uint32_t* h_n_jets,
-                       uint8_t* h_flag, hough_peak* h_peaks, hough_jet* h_jets, float* ms_stage, void* stream)
+int hough_vertices(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks, float d0_cut_mm,
+                   uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices, uint8_t* d_flag,
+                   uint16_t* d_vertex_plane, void* stream)
+{
+    if (!ctx || !d_peaks || !d_n_peaks || !d_vertices || !d_n_vertices || !d_flag) return HOUGH_EINVAL;
+    if (ctx->cfg.n_vtx_phi == 0 || n_events > ctx->cfg.max_events || n_min < 1 || n_min > 65535u || isnan(d0_cut_mm))
+        return HOUGH_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    ctx->last_stream = st;
+    prof_mark(ctx, 4, st);
+    CK(launch_vertices(ctx, n_events, d_peaks, d_n_peaks, d0_cut_mm, n_min, d_vertices, d_n_vertices, d_flag,
+                       d_vertex_plane, st), "vertex kernel");
+    prof_mark(ctx, -1, st);
+    return HOUGH_OK;
+}
+
+int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
+                           const float* h_r, const float* h_phi, const uint8_t* h_layer, uint32_t l_min, float cone_rad,
+                           float d0_cut_mm, uint32_t n_displaced_min, uint32_t vtx_n_min, uint32_t* h_n_peaks,
+                           uint32_t* h_n_jets, uint8_t* h_flag, hough_peak* h_peaks, hough_jet* h_jets,
+                           uint32_t* h_n_vertices, uint8_t* h_vtx_flag, hough_vertex* h_vertices, float* ms_stage,
+                           void* stream)
 {
     if (!ctx || !h_hit_offsets || !h_n_peaks || !h_n_jets || !h_flag) return HOUGH_EINVAL;
     if (ctx->cfg.host_chunk_events == 0) return HOUGH_EINVAL;
@@ -307,9 +359,12 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
     if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
     if (l_min < 1 || l_min > ctx->cfg.n_layers || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm))
         return HOUGH_EINVAL;
+    const bool vtx = vtx_n_min != 0;                            // 0: the second transform is not run
+    if (vtx && (ctx->cfg.n_vtx_phi == 0 || vtx_n_min > 65535u || !h_n_vertices || !h_vtx_flag)) return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
-    if (ms_stage) ms_stage[0] = ms_stage[1] = ms_stage[2] = 0.f;
+    const int n_stage = vtx ? 4 : 3;
+    if (ms_stage) for (int i = 0; i < n_stage; ++i) ms_stage[i] = 0.f;
     if (n_events == 0) return HOUGH_OK;
     const hough_config& g = ctx->cfg;
     CK(cudaMemcpyAsync(ctx->d_hp_off, h_hit_offsets, ((size_t)n_events + 1) * 4, cudaMemcpyHostToDevice, st), "H2D offsets");
@@ -321,10 +376,23 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
     // ms_stage: the context's stage profile (hough_profile) is switched on for this call and read at its end
     const bool prof_was_on = ctx->prof_on;
     if (ms_stage) {
-        float drop[4]; uint32_t nc = 0;
+        float drop[5]; uint32_t nc = 0;
         if (prof_was_on) hough_profile_read(ctx, drop, &nc);     // keep earlier intervals out of this call's numbers
         ctx->prof_on = true;
     }
+    auto peaks_of = [&](uint32_t e) { return ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event; };
+    auto tail = [&](uint32_t e0, uint32_t ne, int cone_bins) -> cudaError_t {   // jets (+ vertices) of events [e0, e0 + ne)
+        prof_mark(ctx, 3, st);
+        cudaError_t err = launch_jets(ctx, ne, peaks_of(e0), ctx->d_hp_npeaks + e0, cone_bins, d0_cut_mm, n_displaced_min,
+                                      ctx->d_hp_tracks + (size_t)e0 * g.max_peaks_per_event,
+                                      ctx->d_hp_jets + (size_t)e0 * g.max_jets_per_event, ctx->d_hp_njets + e0,
+                                      ctx->d_hp_flag + e0, st);
+        if (err != cudaSuccess || !vtx) return err;
+        prof_mark(ctx, 4, st);
+        return launch_vertices(ctx, ne, peaks_of(e0), ctx->d_hp_npeaks + e0, d0_cut_mm, vtx_n_min,
+                               ctx->d_hp_vertices + (size_t)e0 * g.max_vertices_per_event, ctx->d_hp_nvtx + e0,
+                               ctx->d_hp_vflag + e0, nullptr, st);
+    };
     // hits are prepared once for the whole batch; the chunks then share the prepared records
     prof_mark(ctx, 0, st);
     CK(launch_prep(ctx, n_events, ctx->d_hp_off, n_hits_total, ctx->d_hp_r, ctx->d_hp_phi, ctx->d_hp_layer, st), "hit preparation");
@@ -335,13 +403,8 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
         CK(launch_vote_fused(ctx, e0, ne, l_min, st), "fused vote kernel");
         prof_mark(ctx, 2, st);
         CK(launch_recount(ctx, e0, ne, st), "recount kernel");
-        CK(launch_peaks_finalize(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, st),
-           "peak ordering kernel");
-        prof_mark(ctx, 3, st);
-        CK(launch_jets(ctx, ne, ctx->d_hp_peaks + (size_t)e0 * g.max_peaks_per_event, ctx->d_hp_npeaks + e0, cone_bins,
-                       d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e0 * g.max_peaks_per_event,
-                       ctx->d_hp_jets + (size_t)e0 * g.max_jets_per_event, ctx->d_hp_njets + e0, ctx->d_hp_flag + e0, st),
-           "jet kernel");
+        CK(launch_peaks_finalize(ctx, ne, peaks_of(e0), ctx->d_hp_npeaks + e0, st), "peak ordering kernel");
+        CK(tail(e0, ne, cone_bins), "jet / vertex kernels");
     }
     prof_mark(ctx, -1, st);
     CK(cudaMemcpyAsync(h_n_peaks, ctx->d_hp_npeaks, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks");
@@ -351,12 +414,10 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
     for (uint32_t e = 0; e < n_events; ++e) {
         if (h_n_peaks[e] != HOUGH_N_PEAKS_OVERFLOW) continue;
         CK(launch_vote(ctx, e, 1, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel (fallback)");
-        CK(launch_peaks(ctx, 1, ctx->d_hp_count, ctx->d_hp_mask, l_min, ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event,
-                        ctx->d_hp_npeaks + e, st), "peak kernels (fallback)");
-        CK(launch_jets(ctx, 1, ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event, ctx->d_hp_npeaks + e, cone_bins,
-                       d0_cut_mm, n_displaced_min, ctx->d_hp_tracks + (size_t)e * g.max_peaks_per_event,
-                       ctx->d_hp_jets + (size_t)e * g.max_jets_per_event, ctx->d_hp_njets + e, ctx->d_hp_flag + e, st),
-           "jet kernel (fallback)");
+        CK(launch_peaks(ctx, 1, ctx->d_hp_count, ctx->d_hp_mask, l_min, peaks_of(e), ctx->d_hp_npeaks + e, st),
+           "peak kernels (fallback)");
+        CK(tail(e, 1, cone_bins), "jet / vertex kernels (fallback)");
+        prof_mark(ctx, -1, st);
         CK(cudaMemcpyAsync(h_n_peaks + e, ctx->d_hp_npeaks + e, 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks (fallback)");
     }
     CK(cudaMemcpyAsync(h_n_jets, ctx->d_hp_njets, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_jets");
@@ -367,14 +428,32 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
     if (h_jets)
         CK(cudaMemcpyAsync(h_jets, ctx->d_hp_jets, (size_t)n_events * g.max_jets_per_event * sizeof(hough_jet),
                            cudaMemcpyDeviceToHost, st), "D2H jets");
+    if (vtx) {
+        CK(cudaMemcpyAsync(h_n_vertices, ctx->d_hp_nvtx, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_vertices");
+        CK(cudaMemcpyAsync(h_vtx_flag, ctx->d_hp_vflag, (size_t)n_events, cudaMemcpyDeviceToHost, st), "D2H vertex flag");
+        if (h_vertices)
+            CK(cudaMemcpyAsync(h_vertices, ctx->d_hp_vertices, (size_t)n_events * g.max_vertices_per_event * sizeof(hough_vertex),
+                               cudaMemcpyDeviceToHost, st), "D2H vertices");
+    }
     CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
     if (ms_stage) {
-        float ms[4]; uint32_t nc = 0;
+        float ms[5]; uint32_t nc = 0;
         hough_profile_read(ctx, ms, &nc);
         ms_stage[0] = ms[0] + ms[1]; ms_stage[1] = ms[2]; ms_stage[2] = ms[3];
+        if (vtx) ms_stage[3] = ms[4];
         ctx->prof_on = prof_was_on;
     }
     return HOUGH_OK;
+}
+
+int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
+                       const float* h_r, const float* h_phi, const uint8_t* h_layer, uint32_t l_min, float cone_rad,
+                       float d0_cut_mm, uint32_t n_displaced_min, uint32_t* h_n_peaks, uint32_t* h_n_jets,
+                       uint8_t* h_flag, hough_peak* h_peaks, hough_jet* h_jets, float* ms_stage, void* stream)
+{
+    return hough_trigger_host_vtx(ctx, n_events, h_hit_offsets, n_hits_total, h_r, h_phi, h_layer, l_min, cone_rad,
+                                  d0_cut_mm, n_displaced_min, 0u, h_n_peaks, h_n_jets, h_flag, h_peaks, h_jets, nullptr,
+                                  nullptr, nullptr, ms_stage, stream);
 }
 
 int hough_status(hough_ctx* ctx, uint32_t* host_status_bits)
@@ -420,14 +499,14 @@ int hough_profile(hough_ctx* ctx, int enable)
 int hough_profile_read(hough_ctx* ctx, float* h_ms, uint32_t* h_calls)
 {
     if (!ctx || !h_ms) return HOUGH_EINVAL;
-    for (int i = 0; i < 4; ++i) h_ms[i] = 0.f;
+    for (int i = 0; i < 5; ++i) h_ms[i] = 0.f;
     uint32_t calls = 0;
     if (ctx->ev_used) CK(cudaEventSynchronize(ctx->ev_pool[ctx->ev_used - 1]), "hough_profile_read synchronize");
     for (size_t i = 0; i + 1 < ctx->ev_used; ++i) {
         const int label = ctx->ev_label[i];
         if (label < 0) { ++calls; continue; }                  // end of a call: the gap to the next call is nobody's
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, ctx->ev_pool[i], ctx->ev_pool[i + 1]) == cudaSuccess) h_ms[label & 3] += ms;
+        if (cudaEventElapsedTime(&ms, ctx->ev_pool[i], ctx->ev_pool[i + 1]) == cudaSuccess) h_ms[label > 4 ? 4 : label] += ms;
     }
     if (ctx->ev_used) ++calls;
     ctx->ev_used = 0;

@@ -53,6 +53,9 @@ struct hough_ctx {
     float* d_c0; float* d_s0;                 // [NPHI]
     float* d_d0c; float* d_two_d0; float* d_d0sq;   // [ND]
     float kmax, inv_dk, nk_f;
+    float* d_kc;                              // [NK] kappa bin centres, fp32 rounded once from double (O-6)
+    float* d_vex; float* d_vey;               // [n_vtx_phi] phi_v bin-edge directions (cos, sin)(k * 2pi / n_vtx_phi)
+    float* d_vrc;                             // [n_vtx_r] R_v bin centres
     bool tame_tables;                         // d0 centres and kappa_max inside the range div_rn_tame is proven for
     // per-call workspace
     float4* d_rec_u;                          // [max_hits] prepared hits in input order (sort scratch)
@@ -78,10 +81,11 @@ struct hough_ctx {
     uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
     hough_peak* d_hp_peaks; hough_track* d_hp_tracks; hough_jet* d_hp_jets;
     uint32_t* d_hp_npeaks; uint32_t* d_hp_njets; uint8_t* d_hp_flag;
+    hough_vertex* d_hp_vertices; uint32_t* d_hp_nvtx; uint8_t* d_hp_vflag;
     // per-stage CUDA-event timing (hough_profile): marks recorded on the caller's stream around the launches
     bool prof_on;
     std::vector<cudaEvent_t> ev_pool;         // created on first use, reused, freed in hough_destroy
-    std::vector<int> ev_label;                // stage that STARTS at the mark (0 prep, 1 vote, 2 peaks, 3 jets), -1: end of a call
+    std::vector<int> ev_label;                // stage that STARTS at the mark (0 prep, 1 vote, 2 peaks, 3 jets, 4 vertices), -1: end of a call
     size_t ev_used;
     VotePlan vote;
     PeakPlan peak;
@@ -104,6 +108,9 @@ cudaError_t launch_vote_fused(hough_ctx* c, uint32_t first_event, uint32_t n_eve
 cudaError_t launch_recount(hough_ctx* c, uint32_t first_event, uint32_t n_events, cudaStream_t st);
 cudaError_t launch_peaks_finalize(hough_ctx* c, uint32_t n_events, hough_peak* d_peaks, uint32_t* d_n_peaks,
                                   cudaStream_t st);
+cudaError_t launch_vertices(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                            float d0_cut, uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices,
+                            uint8_t* d_flag, uint16_t* d_plane, cudaStream_t st);
 cudaError_t plan_vote(hough_ctx* c);
 cudaError_t plan_peaks(hough_ctx* c);
 cudaError_t run_div_check(uint64_t n_pairs, uint64_t seed, float kmax, int nk, unsigned long long* host_out3);

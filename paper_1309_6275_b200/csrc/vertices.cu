@@ -1,0 +1,196 @@
+// The paper's second Hough transform: tracks -> displaced vertices (sm_100a).
+//
+// PAPER.md:117 (section 6): "the corresponding parameter space representation of these tracks is processed by a
+// second application of the Hough transform ... to identify not straight lines but sinusoids which contain a
+// significant number of tracks, indicating that this is a location of a displaced jet or black hole ... the same
+// peak finding algorithm is applied to the parameter space of this second Hough transform"; the jet of
+// tracks from the interaction point is excluded "by setting a lower bound on the radius"; the cost is
+// proportional to the number of tracks.  Normative arithmetic: DESIGN.md O-6 / O-7 (readings R34-R39).
+//
+// One block per event; the whole vertex accumulator (phi_v x R_v bins, 16-bit counts, two per 32-bit word) lives in
+// shared memory, so nothing but the peak list of the first transform is read and nothing but the vertex list written.
+//   O-6  a warp takes a track (bin-centre parameters d0c, (cos, sin) phi0c, kappa_c of its peak), its lanes the R_v
+//        bins: s = (kappa (r^2 + d0^2) - 2 d0) / (2 r (1 - kappa d0)) with IEEE division, the crossing direction by
+//        rotating (cos phi0, sin phi0) by (sqrt(1 - s^2), s) with IEEE sqrt, the phi_v bin by a cross-product binary
+//        search over the bin-edge directions of the quadrant: no transcendental per vote, every step one IEEE fp32
+//        operation, so the bins are the oracle's.  One shared-memory atomic per vote.
+//   O-7  rule O-3 on the (phi_v, R_v) grid with a count threshold (phi_v periodic, R_v clipped, ties to the lower
+//        linear index), ordered compaction by a block scan over contiguous bin ranges, true total, capacity cut.
+#include "hough_internal.cuh"
+
+namespace {
+
+constexpr int kVtxThreads = 512;
+
+struct VtxParams {
+    const hough_peak* peaks; const uint32_t* n_peaks;
+    hough_vertex* vertices; uint32_t* n_vertices; uint8_t* flag; uint16_t* plane;
+    const float* d0c; const float* c0; const float* s0; const float* kc;      // first transform's bin centres
+    const float* ex; const float* ey; const float* rc;                       // vertex grid: edge directions, R_v centres
+    uint32_t n_events, max_peaks, max_vertices;
+    int n_d0, n_phi0, n_kappa;
+    int n_vphi, n_vr;
+    float d0_cut;
+    uint32_t n_min;
+    double dphi_v;
+};
+
+__device__ __forceinline__ uint32_t angle_bin(const float* __restrict__ ex, const float* __restrict__ ey, int n_vphi, float x,
+                                              float y)
+{
+    uint32_t q;                                  // [0,pi/2): x>0,y>=0   [pi/2,pi): x<=0,y>0   [pi,3pi/2): x<0,y<=0   else
+    if (x > 0.0f && y >= 0.0f) q = 0u;
+    else if (x <= 0.0f && y > 0.0f) q = 1u;
+    else if (x < 0.0f && y <= 0.0f) q = 2u;
+    else q = 3u;
+    uint32_t lo = q * ((uint32_t)n_vphi / 4u), hi = lo + (uint32_t)n_vphi / 4u - 1u;
+    while (lo < hi) {
+        const uint32_t mid = (lo + hi + 1u) / 2u;
+        const float cr = __fsub_rn(__fmul_rn(ex[mid], y), __fmul_rn(ey[mid], x));
+        if (cr >= 0.0f) lo = mid; else hi = mid - 1u;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ uint32_t vcount(const uint32_t* acc, uint32_t b)
+{
+    return (acc[b >> 1] >> (16u * (b & 1u))) & 0xffffu;
+}
+
+// O-3 on the vertex plane for bin (iv, ir) with count c >= n_min
+__device__ __forceinline__ bool vtx_is_peak(const uint32_t* acc, int NPV, int NR, int iv, int ir, uint32_t c)
+{
+    const uint32_t lin = (uint32_t)iv * (uint32_t)NR + (uint32_t)ir;
+#pragma unroll
+    for (int dp = -1; dp <= 1; ++dp) {
+        int jv = iv + dp;
+        jv = (jv < 0) ? jv + NPV : (jv >= NPV ? jv - NPV : jv);
+#pragma unroll
+        for (int dr = -1; dr <= 1; ++dr) {
+            if (dp == 0 && dr == 0) continue;
+            const int jr = ir + dr;
+            if (jr < 0 || jr >= NR) continue;
+            const uint32_t nl = (uint32_t)jv * (uint32_t)NR + (uint32_t)jr;
+            const uint32_t cn = vcount(acc, nl);
+            if (!(c > cn || (c == cn && lin < nl))) return false;
+        }
+    }
+    return true;
+}
+
+__global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
+{
+    extern __shared__ uint32_t acc[];                            // [n_vphi * n_vr / 2]: two 16-bit counts per word
+    __shared__ uint32_t s_warp[kVtxThreads / 32];
+    __shared__ uint32_t s_total;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t e = blockIdx.x;
+    const int NPV = p.n_vphi, NR = p.n_vr;
+    const uint32_t bins = (uint32_t)NPV * (uint32_t)NR;
+    for (uint32_t i = tid; i < bins / 2; i += kVtxThreads) acc[i] = 0u;
+    __syncthreads();
+
+    const uint32_t np_e = p.n_peaks[e];
+    const uint32_t T = (np_e == HOUGH_N_PEAKS_OVERFLOW) ? 0u : min(np_e, p.max_peaks);
+    const hough_peak* pk = p.peaks + (size_t)e * p.max_peaks;
+    // ---- O-6: one warp per track, lanes over the R_v bins ----
+    for (uint32_t j = warp; j < T; j += kVtxThreads / 32) {
+        const uint32_t lin = pk[j].lin;
+        const uint32_t ik = lin % (uint32_t)p.n_kappa, t = lin / (uint32_t)p.n_kappa;
+        const uint32_t ip = t % (uint32_t)p.n_phi0, id = t / (uint32_t)p.n_phi0;
+        const float d0 = (p.n_d0 > 1) ? __ldg(p.d0c + id) : 0.0f;
+        if (!(fabsf(d0) > p.d0_cut)) continue;                   // prompt-compatible track: does not vote (warp-uniform)
+        const float c0 = __ldg(p.c0 + ip), s0 = __ldg(p.s0 + ip), kap = __ldg(p.kc + ik);
+        const float kd = __fmul_rn(kap, d0);
+        const float w = __fsub_rn(1.0f, kd);
+        const float d2 = __fmul_rn(d0, d0);
+        const float two_d0 = __fadd_rn(d0, d0);
+        for (int ir = lane; ir < NR; ir += 32) {
+            const float r = __ldg(p.rc + ir);
+            const float r2 = __fmul_rn(r, r);
+            const float num = __fsub_rn(__fmul_rn(kap, __fadd_rn(r2, d2)), two_d0);
+            const float den = __fmul_rn(__fadd_rn(r, r), w);
+            const float s = __fdiv_rn(num, den);
+            if (!(fabsf(s) <= 1.0f)) continue;                   // the track does not reach this radius
+            const float cd = __fsqrt_rn(__fsub_rn(1.0f, __fmul_rn(s, s)));
+            const float x = __fsub_rn(__fmul_rn(c0, cd), __fmul_rn(s0, s));
+            const float y = __fadd_rn(__fmul_rn(s0, cd), __fmul_rn(c0, s));
+            const uint32_t b = angle_bin(p.ex, p.ey, NPV, x, y) * (uint32_t)NR + (uint32_t)ir;
+            atomicAdd(&acc[b >> 1], 1u << (16u * (b & 1u)));
+        }
+    }
+    __syncthreads();
+    if (p.plane) {                                               // optional: the vertex plane itself (tests)
+        uint32_t* out = reinterpret_cast<uint32_t*>(p.plane + (size_t)e * bins);
+        for (uint32_t i = tid; i < bins / 2; i += kVtxThreads) out[i] = acc[i];
+    }
+    // ---- O-7: peaks in ascending linear index: each thread owns a contiguous range of bins ----
+    const uint32_t per = (bins + kVtxThreads - 1) / kVtxThreads;
+    const uint32_t b_lo = min((uint32_t)tid * per, bins), b_hi = min(b_lo + per, bins);
+    uint32_t mine = 0;
+    for (uint32_t b = b_lo; b < b_hi; ++b) {
+        const uint32_t c = vcount(acc, b);
+        if (c >= p.n_min && vtx_is_peak(acc, NPV, NR, (int)(b / (uint32_t)NR), (int)(b % (uint32_t)NR), c)) ++mine;
+    }
+    uint32_t incl = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t wsum = (lane < kVtxThreads / 32) ? s_warp[lane] : 0u;
+        uint32_t winc = wsum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += t;
+        }
+        if (lane < kVtxThreads / 32) s_warp[lane] = winc - wsum;
+        if (lane == 31) s_total = winc;
+    }
+    __syncthreads();
+    uint32_t pos = s_warp[warp] + incl - mine;
+    hough_vertex* out = p.vertices + (size_t)e * p.max_vertices;
+    if (mine > 0 && pos < p.max_vertices) {
+        for (uint32_t b = b_lo; b < b_hi && pos < p.max_vertices; ++b) {
+            const uint32_t c = vcount(acc, b);
+            const int iv = (int)(b / (uint32_t)NR), ir = (int)(b % (uint32_t)NR);
+            if (c >= p.n_min && vtx_is_peak(acc, NPV, NR, iv, ir, c)) {
+                hough_vertex vx;
+                vx.r = p.rc[ir];
+                vx.phi = (float)(((double)iv + 0.5) * p.dphi_v);
+                vx.n_tracks = c; vx.lin = b;
+                out[pos++] = vx;
+            }
+        }
+    }
+    if (tid == 0) { p.n_vertices[e] = s_total; p.flag[e] = s_total > 0u ? 1 : 0; }
+}
+
+}  // namespace
+
+cudaError_t launch_vertices(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                            float d0_cut, uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices,
+                            uint8_t* d_flag, uint16_t* d_plane, cudaStream_t st)
+{
+    if (n_events == 0) return cudaSuccess;
+    VtxParams p;
+    p.peaks = d_peaks; p.n_peaks = d_n_peaks; p.vertices = d_vertices; p.n_vertices = d_n_vertices; p.flag = d_flag;
+    p.plane = d_plane;
+    p.d0c = c->d_d0c; p.c0 = c->d_c0; p.s0 = c->d_s0; p.kc = c->d_kc;
+    p.ex = c->d_vex; p.ey = c->d_vey; p.rc = c->d_vrc;
+    p.n_events = n_events; p.max_peaks = c->cfg.max_peaks_per_event; p.max_vertices = c->cfg.max_vertices_per_event;
+    p.n_d0 = (int)c->cfg.n_d0; p.n_phi0 = (int)c->cfg.n_phi0; p.n_kappa = (int)c->cfg.n_kappa;
+    p.n_vphi = (int)c->cfg.n_vtx_phi; p.n_vr = (int)c->cfg.n_vtx_r;
+    p.d0_cut = d0_cut; p.n_min = n_min;
+    p.dphi_v = 6.283185307179586476925286766559 / (double)c->cfg.n_vtx_phi;
+    const size_t smem = (size_t)c->cfg.n_vtx_phi * c->cfg.n_vtx_r * 2;
+    cudaError_t err = cudaFuncSetAttribute(vertex_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (err != cudaSuccess) return err;
+    vertex_kernel<<<n_events, kVtxThreads, smem, st>>>(p);
+    ++c->launches;
+    return cudaGetLastError();
+}

@@ -54,6 +54,13 @@ class Workload:
     cone_rad: float = 0.4
     d0_cut_mm: float = 2.0
     n_displaced_min: int = 3
+    # vertex space of the second Hough transform (beam pipe 30 mm) and its threshold
+    vtx_n_phi: int = 256
+    vtx_n_r: int = 128
+    vtx_r_min: float = 30.0
+    vtx_r_max: float = 430.0
+    vtx_n_min: int = 4
+    max_vertices: int = 64
     # event content
     n_prompt: Tuple[int, int] = (10, 10)            # inclusive integer range
     prompt_pt: str = "uniform_1_20"                 # or "exp2_trunc1"
@@ -72,6 +79,10 @@ class Workload:
     @property
     def bins_per_event(self) -> int:
         return self.n_d0 * self.n_phi0 * self.n_kappa
+
+    @property
+    def vgrid(self):
+        return (self.vtx_n_phi, self.vtx_n_r, self.vtx_r_min, self.vtx_r_max)
 
 
 def config(k: int) -> Workload:

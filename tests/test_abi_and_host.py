@@ -38,9 +38,9 @@ def test_strerror_and_argument_validation_without_gpu():
     assert B.strerror(0) == "ok" and "invalid" in B.strerror(-1)
     # a bad config is rejected before any CUDA call; null pointers likewise
     ctx = C.c_void_p()
-    bad = B.HoughConfig(512, 250, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0)       # n_kappa % 8 != 0
+    bad = B.HoughConfig(512, 250, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0)       # n_kappa % 8 != 0
     assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
-    bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0, 0)     # n_layers > 16
+    bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0)     # n_layers > 16
     assert lib.hough_create(C.byref(bad2), C.byref(ctx)) == -1
     assert lib.hough_create(None, C.byref(ctx)) == -1
     assert lib.hough_destroy(None) == -1
@@ -56,7 +56,9 @@ def test_config_struct_layout_matches_header():
     #include "hough.h"
     int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(hough_config), offsetof(hough_config, max_hits),
         offsetof(hough_config, host_chunk_events), sizeof(hough_peak), sizeof(hough_track), sizeof(hough_jet),
-        offsetof(hough_config, max_events), offsetof(hough_config, max_candidates_per_event)); return 0; }'''
+        offsetof(hough_config, max_events), offsetof(hough_config, max_candidates_per_event));
+        printf("%zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex));
+        return 0; }'''
     exe = os.path.join(ROOT, "_work", "layout_probe") if os.path.isdir(os.path.join(ROOT, "_work")) else "/tmp/layout_probe"
     exe = "/tmp/hough_layout_probe"
     subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=src, text=True, check=True)
@@ -64,6 +66,8 @@ def test_config_struct_layout_matches_header():
     assert vals[0] == C.sizeof(B.HoughConfig)
     assert vals[1] == B.HoughConfig.max_hits.offset and vals[2] == B.HoughConfig.host_chunk_events.offset
     assert vals[6] == B.HoughConfig.max_events.offset and vals[7] == B.HoughConfig.max_candidates_per_event.offset
+    assert vals[8] == B.HoughConfig.vtx_r_min.offset and vals[9] == B.HoughConfig.max_vertices_per_event.offset
+    assert vals[10] == B.VERTEX_DTYPE.itemsize == 16
     assert vals[3] == B.PEAK_DTYPE.itemsize == 8 and vals[4] == B.TRACK_DTYPE.itemsize == 20
     assert vals[5] == B.JET_DTYPE.itemsize == 20
 
