@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- whole hot path (vote -> peaks -> tracks -> jets) on synthetic trigger batches, one JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3|C2|C1] [--events E]
-                  [--path fused|planes] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3|C2|C1|P4] [--events E]
+                  [--path fused|planes] [--impl ours|reference] [--tracks N]
 
 A "step" is one pass of the whole hot path over one batch (BASELINE.json configs[4] by default: 4,096 events,
 12-layer tracker, 128 x 1024 x 512 accumulator per event, processed in launches of --chunk events).  The default
@@ -203,6 +203,8 @@ def traffic_from_profiles(kernel_substr: str):
 
 def make_workload(name: str, n_events):
     from paper_1309_6275_b200 import workloads as W
+    if name == "P4":
+        return W.paper_timing(3000, int(n_events) if n_events else 32)
     k = {"C1": 1, "C2": 2, "C3": 3, "C4": 4, "C5": 5}[name]
     w = W.config(k)
     if n_events:
@@ -436,6 +438,84 @@ def measure_config(name: str, hbm_gbs, sm_max_mhz, peak_src, steps: int = 3):
     return res
 
 
+def run_p4(args):
+    """--workload P4: the paper's own timing benchmark (Fig. 4): time per event against tracks per
+    event on the ten-layer toy detector with a 2048 x 2048 accumulator, fused path, one launch per batch."""
+    import torch
+    from paper_1309_6275_b200 import binding as B
+    from paper_1309_6275_b200 import workloads as W
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1 or args.gpus != 1:
+        raise SystemExit("bench.py --workload P4 is a single-GPU curve")
+    torch.cuda.set_device(0)
+    hbm_gbs, sm_max_mhz, peak_src = measured_peaks()
+    points = [args.tracks] if args.tracks else [100, 300, 1000, 3000]
+    E = args.events or 32
+    curve, last = [], None
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    wall0 = time.time()
+    for n in points:
+        w = W.paper_timing(n, E)
+        batch = W.generate(w)
+        votes = count_votes(w, batch)
+        d = {"tracks_per_event": n, "hits_per_event": batch.n_hits // E, "votes_per_event": votes / E}
+        for path in ("fused", "planes"):
+            run = DeviceRun(w, batch, E, path, vertices=False)
+            ms, stage, launches = run.timed(args.steps, args.warmup)
+            d[path] = {"ms_per_event": ms / args.steps / E, "events_per_sec": E * args.steps / (ms * 1e-3),
+                       "stage_ms_per_event": {k: v / args.steps / E for k, v in zip(STAGES, stage)},
+                       "roofline": vote_roofline("2d", votes * args.steps, 0 if path == "fused" else w.bins_per_event * E * args.steps,
+                                                 stage[1], args.steps, hbm_gbs, sm_max_mhz, peak_src,
+                                                 "vote_kernel<fused>" if path == "fused" else "vote_kernel")}
+            if path == "fused":
+                d["peaks_per_event"] = float(run.out["n_peaks"].float().mean().item())
+                last = (w, batch, ms, stage, launches, votes)
+            run.close()
+            torch.cuda.empty_cache()
+        curve.append(d)
+    wall1 = time.time()
+    clocks = sampler.stop(wall0, wall1)
+    w, batch, ms, stage, launches, votes = last
+    H = batch.n_hits
+    # e2e at the last point
+    h2 = B.Hough.for_workload(w, max_events=E, max_hits=H, host_chunk_events=E)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    h_off, h_r, h_phi, h_layer = pin(batch.hit_offsets.view(np.int32)), pin(batch.r), pin(batch.phi), pin(batch.layer)
+    h_np = torch.zeros(E, dtype=torch.int32).pin_memory(); h_nj = torch.zeros(E, dtype=torch.int32).pin_memory()
+    h_fl = torch.zeros(E, dtype=torch.uint8).pin_memory()
+    h_pk = torch.zeros((E, w.max_peaks, 8), dtype=torch.uint8).pin_memory()
+    stream = torch.cuda.current_stream()
+    call = lambda: h2.hough_trigger_host(E, h_off, H, h_r, h_phi, h_layer, w.l_min, w.cone_rad, w.d0_cut_mm,
+                                         w.n_displaced_min, h_np, h_nj, h_fl, h_pk, None, None, stream)
+    call(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(args.steps): call()
+    b.record(stream); torch.cuda.synchronize()
+    e2e_value = E * args.steps / (a.elapsed_time(b) * 1e-3)
+    h2_launches = h2.hough_launch_count()
+    h2.close()
+    cpu = cpu_oracle_rate(w, batch, budget_s=10.0) if not args.no_cpu_baseline else None
+    line = {"metric": "events_per_sec", "value": E * args.steps / (ms * 1e-3), "unit": "events/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "path": "fused", "events_per_gpu": E, "hits": H,
+                       "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min,
+                       "detector": "PAPER.md:97-99: beam pipe 30 mm, 10 layers evenly spaced to 1100 mm, 0.4 mm resolution",
+                       "l2": "no L2 flush needed: compute-bound, no planes in HBM on the fused path",
+                       "note": "paper's Fig. 4 workload; its absolute times are in an unreadable figure (context only)"},
+            "curve_time_vs_tracks": curve, "votes_per_step": votes, "clocks": clocks,
+            "stage_ms_per_step": {k: v / args.steps for k, v in zip(STAGES, stage)},
+            "e2e": {"value": e2e_value, "unit": "events/s", "h2d_bytes_per_step": int(H * 9 + (E + 1) * 4),
+                    "d2h_bytes_per_step": int(E * 9 + E * w.max_peaks * 8), "steps": args.steps},
+            "gpu_launches": int(launches), "gpu_launches_e2e": int(h2_launches),
+            "roofline": curve[-1]["fused"]["roofline"]}
+    if cpu:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line))
+
+
 def run_ours(args):
     import torch
     from paper_1309_6275_b200 import binding as B
@@ -624,7 +704,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "P4"])
+    ap.add_argument("--tracks", type=int, default=0, help="P4 only: one point of the curve (0 = 100, 300, 1000, 3000)")
     ap.add_argument("--path", default="fused", choices=["fused", "planes"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (0 = the config's)")
     ap.add_argument("--chunk", type=int, default=0, help="events per launch (0: what would fit in 34 GB of planes)")
@@ -638,7 +719,10 @@ def main():
         return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         reexec_under_torchrun(args, sys.argv[1:])
-    run_ours(args)
+    if args.workload == "P4":
+        run_p4(args)
+    else:
+        run_ours(args)
 
 
 if __name__ == "__main__":

@@ -175,7 +175,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_rec_u, cfg->max_hits)); A(dev_alloc(&c->d_key, cfg->max_hits));
     A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
     A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
-    A(dev_alloc(&c->d_layer_r, 2 * HOUGH_MAX_LAYERS));
+    A(dev_alloc(&c->d_layer_r, 4 * HOUGH_MAX_LAYERS));   // live min / max per layer + the copy the recount reads
     A(dev_alloc(&c->d_tilewin, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_tilectr, 2));
@@ -215,8 +215,11 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         cudaGetLastError();
         return (err == cudaErrorMemoryAllocation) ? HOUGH_ENOMEM : HOUGH_ECUDA;
     }
-    uint32_t lr[2 * HOUGH_MAX_LAYERS];
-    for (int i = 0; i < HOUGH_MAX_LAYERS; ++i) { lr[i] = 0x7f800000u; lr[HOUGH_MAX_LAYERS + i] = 0u; }
+    uint32_t lr[4 * HOUGH_MAX_LAYERS];
+    for (int i = 0; i < HOUGH_MAX_LAYERS; ++i) {
+        lr[i] = lr[2 * HOUGH_MAX_LAYERS + i] = 0x7f800000u;
+        lr[HOUGH_MAX_LAYERS + i] = lr[3 * HOUGH_MAX_LAYERS + i] = 0u;
+    }
     A(cudaMemcpy(c->d_c0, c0.data(), NP * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_s0, s0.data(), NP * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_d0c, d0c.data(), ND * 4, cudaMemcpyHostToDevice));

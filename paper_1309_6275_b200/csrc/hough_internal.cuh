@@ -63,7 +63,7 @@ struct hough_ctx {
     float4* d_rec;                            // [max_hits] prepared hits sorted per event by (layer, phi bucket)
     uint32_t* d_seg;                          // [max_events][kSegStride]
     uint16_t* d_btab;                         // [max_events][16][nb + 1] bucket starts relative to the layer segment
-    uint32_t* d_layer_r;                      // [2*16] float bits: min r, max r per layer
+    uint32_t* d_layer_r;                      // [4*16] float bits: min r, max r per layer (live), then the last call's copy
     TileWin* d_tilewin;                       // [nk_seg][16][n_strips]
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
     uint32_t* d_tilectr;                      // [2]: vote kernel tile ticket + finished-block count (zero between launches)

@@ -28,6 +28,9 @@ TWO_PI = 2.0 * np.pi
 
 TRACKER_A = (40.0, 70.0, 110.0, 250.0, 330.0, 430.0, 520.0, 600.0)            # 8 barrel layers, mm
 TRACKER_B = TRACKER_A + (700.0, 800.0, 900.0, 1000.0)                          # 12 layers
+# the paper's toy detector (section 5): beam pipe of radius 30 mm, ten concentric evenly spaced layers,
+# overall radius 1100 mm, hit resolution 0.4 mm
+TRACKER_PAPER = tuple(30.0 + (i + 1) * (1100.0 - 30.0) / 10.0 for i in range(10))
 B_TESLA = 3.8
 KAPPA_MAX = 0.3e-3 * B_TESLA / 1.0        # |kappa| of a 1 GeV track, 1/mm  (configs: "0.3*3.8/1 GeV per m")
 
@@ -71,6 +74,7 @@ class Workload:
     llp_tracks: Tuple[int, int] = (4, 4)
     llp_pt: Tuple[float, float] = (1.0, 10.0)
     llp_half_angle: float = 0.3
+    hit_sigma_mm: float = 0.02                      # azimuthal smearing of a hit: N(0,1) * hit_sigma_mm / r  (R27)
 
     @property
     def n_layers(self) -> int:
@@ -107,6 +111,15 @@ def config(k: int) -> Workload:
                         n_llp=(1, 4), llp_prob=0.10, llp_radius=(5.0, 400.0), llp_tracks=(6, 12),
                         llp_pt=(1.0, 30.0))
     raise ValueError("config index must be 1..5")
+
+
+def paper_timing(n_tracks: int, n_events: int = 32) -> Workload:
+    """"P4": the paper's own timing benchmark (Fig. 4 "Time vs. tracks per event, 2048x2048"): the
+    ten-layer toy detector, 0.4 mm hit resolution, a 2048 x 2048 (phi0 x kappa) prompt accumulator, n_tracks tracks of
+    10 hits each per event (the paper's curve runs to 3,000 tracks), no noise hits; the peak finder
+    expects "7 or more hits per track".  pT is not stated: 1 + Exp(2) GeV as in the other configs."""
+    return Workload(f"P4-{n_tracks}", 40, n_events, TRACKER_PAPER, 1, 2048, 2048, l_min=7, max_peaks=16384,
+                    n_prompt=(n_tracks, n_tracks), prompt_pt="exp2_trunc1", n_noise=(0, 0), hit_sigma_mm=0.4)
 
 
 def scaled(w: Workload, **kw) -> Workload:
@@ -255,7 +268,7 @@ def generate_event(w: Workload, k: int, seed: Optional[int] = None):
     truth["n_vertices"] = n_v
 
     r_sig = np.concatenate(rs); p_sig = np.concatenate(phis); l_sig = np.concatenate(lays)
-    p_sig = p_sig + rng.standard_normal(p_sig.size) * (0.02 / r_sig)            # R27
+    p_sig = p_sig + rng.standard_normal(p_sig.size) * (w.hit_sigma_mm / r_sig)   # R27
 
     n_n = _randint_incl(rng, w.n_noise)
     l_n = rng.integers(0, radii.size, n_n)
