@@ -2,6 +2,7 @@
 // launches.  No compute happens on the host; there is no CPU fallback.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -123,7 +124,6 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     c->cfg = *cfg;
     c->device = dev;
     c->sm_count = prop.multiProcessorCount;
-    if (plan_vote(c) != cudaSuccess || plan_peaks(c) != cudaSuccess) { delete c; return HOUGH_EUNSUPPORTED; }
 
     // O-0 tables: double precision, each value rounded once to fp32
     const uint32_t NP = cfg->n_phi0, ND = cfg->n_d0, NK = cfg->n_kappa;
@@ -155,6 +155,12 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
             vrc[ir] = (float)((double)cfg->vtx_r_min +
                               ((double)ir + 0.5) * (((double)cfg->vtx_r_max - (double)cfg->vtx_r_min) / (double)cfg->n_vtx_r));
     }
+    // mirror tiles need tables that are antisymmetric bit for bit: c0[ip + N/2] == -c0[ip], s0 likewise, d0c[ND-1-id] == -d0c[id]
+    bool mirror_ok = NP % 2 == 0 && getenv("HOUGH_NO_MIRROR") == nullptr;
+    for (uint32_t ip = 0; mirror_ok && ip < NP / 2; ++ip)
+        mirror_ok = c0[ip + NP / 2] == -c0[ip] && s0[ip + NP / 2] == -s0[ip];
+    for (uint32_t id = 0; mirror_ok && id < ND; ++id) mirror_ok = d0c[ND - 1 - id] == -d0c[id];
+    if (plan_vote(c, mirror_ok) != cudaSuccess || plan_peaks(c) != cudaSuccess) { delete c; return HOUGH_EUNSUPPORTED; }
     // the branch-free exact division of the vote kernel is only used inside this range (vote.cu, div_rn_tame)
     c->tame_tables = cfg->kappa_max >= 9.094947e-13f && cfg->kappa_max <= 1.0995116e12f;      // [2^-40, 2^40]
     for (uint32_t id = 0; id < ND; ++id) {

@@ -36,7 +36,8 @@ struct VotePlan {
     int nk_seg;
     int threads;
     size_t smem_bytes;
-    int n_strips, n_tiles;           // ceil(ND/K), ceil(NPHI/W)
+    int n_strips, n_tiles;           // ceil(ND/K), ceil(NPHI/W)  (mirror: (NPHI/2)/W)
+    bool mirror;                     // mirror tiles: each (hit, row) evaluation also votes the row's mirror image
 };
 
 struct PeakPlan {
@@ -111,6 +112,6 @@ cudaError_t launch_peaks_finalize(hough_ctx* c, uint32_t n_events, hough_peak* d
 cudaError_t launch_vertices(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
                             float d0_cut, uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices,
                             uint8_t* d_flag, uint16_t* d_plane, cudaStream_t st);
-cudaError_t plan_vote(hough_ctx* c);
+cudaError_t plan_vote(hough_ctx* c, bool mirror_ok);
 cudaError_t plan_peaks(hough_ctx* c);
 cudaError_t run_div_check(uint64_t n_pairs, uint64_t seed, float kmax, int nk, unsigned long long* host_out3);

@@ -81,16 +81,23 @@ def test_packed_sweep_keeps_every_rounding_of_o2():
     lib = build.build()
     sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
     kernels = [b for b in sass.split("Function : ")[1:] if "vote_kernelILb1E" in b.split("\n")[0]]
-    assert len(kernels) == 6                                     # KL = 1, 2, 4 x {planes, fused}
+    assert len(kernels) == 8                                     # KL = 1, 2, 4 x {planes, fused} + the two mirror kernels
+    n_mirror = 0
     for body in kernels:
+        mirror = re.search(r"Lb([01])EEEvNS", body.split("\n")[0]).group(1) == "1"     # ..., bool MIRROR>
         n_rm = len(re.findall(r"\bFADD2\.RM\b", body))
         n_add = len(re.findall(r"\bFADD2 ", body))
         n_mul = len(re.findall(r"\bFMUL2 ", body))
         n_fma = len(re.findall(r"\bFFMA2 ", body))
         assert n_rm > 0
-        assert n_add == 3 * n_rm, (n_add, n_rm)
-        assert n_mul == 2 * n_rm, (n_mul, n_rm)
-        assert n_fma == 5 * n_rm, (n_fma, n_rm)
+        if mirror:                                               # per hit pair: 2 floors (row + mirror row), t, b, den,
+            n_mirror += 1                                        # NQ0 + two u, the division's 4 FFMA2 + two v
+            assert 2 * n_add == 3 * n_rm and 2 * n_mul == 3 * n_rm and n_fma == 3 * n_rm, (n_add, n_mul, n_fma, n_rm)
+        else:
+            assert n_add == 3 * n_rm, (n_add, n_rm)
+            assert n_mul == 2 * n_rm, (n_mul, n_rm)
+            assert n_fma == 5 * n_rm, (n_fma, n_rm)
+    assert n_mirror == 2
 
 
 def test_product_path_never_touches_the_oracle():
