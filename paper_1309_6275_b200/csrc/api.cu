@@ -84,6 +84,8 @@ bool config_ok(const hough_config* g)
     if (g->n_vtx_phi != 0) {                                   // vertex grid of the second transform
         if (g->n_vtx_phi < 8 || g->n_vtx_phi % 4 != 0 || g->n_vtx_r < 8 || g->n_vtx_r % 8 != 0) return false;
         if ((uint64_t)g->n_vtx_phi * g->n_vtx_r * 2 > 200u * 1024u) return false;
+        if ((uint64_t)g->n_vtx_phi * g->n_vtx_r * 2 + (2ull * g->n_vtx_phi + g->n_vtx_r) * 4 +
+                (uint64_t)g->n_vtx_phi * g->n_vtx_r / 8 > 220u * 1024u) return false;
         if (!(g->vtx_r_min > 0.f) || !(g->vtx_r_max > g->vtx_r_min) || !isfinite(g->vtx_r_max)) return false;
         if (g->max_vertices_per_event < 1) return false;
     }

@@ -32,17 +32,22 @@ __device__ __forceinline__ uint64_t warp_min_u64(uint64_t v)
     return v;
 }
 
-__global__ void __launch_bounds__(128) jets_kernel(const JetParams p)
+// one warp (= one block) per event; the clustering keys live in shared memory when the event's tracks fit
+// (kSmemKeys of them), else in the context's global workspace
+constexpr uint32_t kSmemKeys = 4096;
+
+__global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
 {
+    __shared__ uint64_t s_keys[kSmemKeys];
     const int lane = threadIdx.x & 31;
-    const uint32_t e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const uint32_t e = blockIdx.x;
     if (e >= p.n_events) return;
     const uint32_t np_e = p.n_peaks[e];
     const uint32_t T = (np_e == HOUGH_N_PEAKS_OVERFLOW) ? 0u : min(np_e, p.max_peaks);   // overflowed fused event: no tracks
     const hough_peak* pk = p.peaks + (size_t)e * p.max_peaks;
     hough_track* trk = p.tracks + (size_t)e * p.max_peaks;
     hough_jet* jets = p.jets + (size_t)e * p.max_jets;
-    uint64_t* keys = p.keys + (size_t)e * p.max_peaks;
+    uint64_t* keys = (T <= kSmemKeys) ? s_keys : p.keys + (size_t)e * p.max_peaks;
     const int NK = p.n_kappa, N = p.n_phi0;
     const double kmax = (double)p.kmax;
 
@@ -130,8 +135,7 @@ cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_pea
     p.n_events = n_events; p.max_peaks = c->cfg.max_peaks_per_event; p.max_jets = c->cfg.max_jets_per_event;
     p.n_d0 = (int)c->cfg.n_d0; p.n_phi0 = (int)c->cfg.n_phi0; p.n_kappa = (int)c->cfg.n_kappa;
     p.kmax = c->kmax; p.b_tesla = c->cfg.b_tesla; p.d0_cut = d0_cut; p.cone_bins = cone_bins; p.n_min = n_min;
-    const uint32_t warps_per_block = 4;
-    jets_kernel<<<(n_events + warps_per_block - 1) / warps_per_block, warps_per_block * 32, 0, st>>>(p);
+    jets_kernel<<<n_events, 32, 0, st>>>(p);
     ++c->launches;
     return cudaGetLastError();
 }

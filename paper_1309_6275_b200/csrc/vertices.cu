@@ -15,7 +15,8 @@
 //        search over the bin-edge directions of the quadrant: no transcendental per vote, every step one IEEE fp32
 //        operation, so the bins are the oracle's.  One shared-memory atomic per vote.
 //   O-7  rule O-3 on the (phi_v, R_v) grid with a count threshold (phi_v periodic, R_v clipped, ties to the lower
-//        linear index), ordered compaction by a block scan over contiguous bin ranges, true total, capacity cut.
+//        linear index): a ballot per chunk of 32 bins, then a block scan of the popcounts for the ordered
+//        compaction; true total, capacity cut.
 #include "hough_internal.cuh"
 
 namespace {
@@ -35,8 +36,7 @@ struct VtxParams {
     double dphi_v;
 };
 
-__device__ __forceinline__ uint32_t angle_bin(const float* __restrict__ ex, const float* __restrict__ ey, int n_vphi, float x,
-                                              float y)
+__device__ __forceinline__ uint32_t angle_bin(const float* ex, const float* ey, int n_vphi, float x, float y)
 {
     uint32_t q;                                  // [0,pi/2): x>0,y>=0   [pi/2,pi): x<=0,y>0   [pi,3pi/2): x<0,y<=0   else
     if (x > 0.0f && y >= 0.0f) q = 0u;
@@ -80,14 +80,20 @@ __device__ __forceinline__ bool vtx_is_peak(const uint32_t* acc, int NPV, int NR
 
 __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
 {
-    extern __shared__ uint32_t acc[];                            // [n_vphi * n_vr / 2]: two 16-bit counts per word
+    extern __shared__ uint32_t acc[];                            // [n_vphi * n_vr / 2]: two 16-bit counts per word, then tables
     __shared__ uint32_t s_warp[kVtxThreads / 32];
     __shared__ uint32_t s_total;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t e = blockIdx.x;
     const int NPV = p.n_vphi, NR = p.n_vr;
     const uint32_t bins = (uint32_t)NPV * (uint32_t)NR;
+    // the edge directions (binary-searched per vote) and the R_v centres live in shared memory behind the accumulator
+    float* s_ex = reinterpret_cast<float*>(acc + bins / 2);
+    float* s_ey = s_ex + NPV;
+    float* s_rc = s_ey + NPV;
     for (uint32_t i = tid; i < bins / 2; i += kVtxThreads) acc[i] = 0u;
+    for (int i = tid; i < NPV; i += kVtxThreads) { s_ex[i] = p.ex[i]; s_ey[i] = p.ey[i]; }
+    for (int i = tid; i < NR; i += kVtxThreads) s_rc[i] = p.rc[i];
     __syncthreads();
 
     const uint32_t np_e = p.n_peaks[e];
@@ -106,7 +112,7 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
         const float d2 = __fmul_rn(d0, d0);
         const float two_d0 = __fadd_rn(d0, d0);
         for (int ir = lane; ir < NR; ir += 32) {
-            const float r = __ldg(p.rc + ir);
+            const float r = s_rc[ir];
             const float r2 = __fmul_rn(r, r);
             const float num = __fsub_rn(__fmul_rn(kap, __fadd_rn(r2, d2)), two_d0);
             const float den = __fmul_rn(__fadd_rn(r, r), w);
@@ -115,7 +121,7 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
             const float cd = __fsqrt_rn(__fsub_rn(1.0f, __fmul_rn(s, s)));
             const float x = __fsub_rn(__fmul_rn(c0, cd), __fmul_rn(s0, s));
             const float y = __fadd_rn(__fmul_rn(s0, cd), __fmul_rn(c0, s));
-            const uint32_t b = angle_bin(p.ex, p.ey, NPV, x, y) * (uint32_t)NR + (uint32_t)ir;
+            const uint32_t b = angle_bin(s_ex, s_ey, NPV, x, y) * (uint32_t)NR + (uint32_t)ir;
             atomicAdd(&acc[b >> 1], 1u << (16u * (b & 1u)));
         }
     }
@@ -124,14 +130,24 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
         uint32_t* out = reinterpret_cast<uint32_t*>(p.plane + (size_t)e * bins);
         for (uint32_t i = tid; i < bins / 2; i += kVtxThreads) out[i] = acc[i];
     }
-    // ---- O-7: peaks in ascending linear index: each thread owns a contiguous range of bins ----
-    const uint32_t per = (bins + kVtxThreads - 1) / kVtxThreads;
-    const uint32_t b_lo = min((uint32_t)tid * per, bins), b_hi = min(b_lo + per, bins);
-    uint32_t mine = 0;
-    for (uint32_t b = b_lo; b < b_hi; ++b) {
-        const uint32_t c = vcount(acc, b);
-        if (c >= p.n_min && vtx_is_peak(acc, NPV, NR, (int)(b / (uint32_t)NR), (int)(b % (uint32_t)NR), c)) ++mine;
+    // ---- O-7: peaks in ascending linear index ----
+    // pass 1: chunks of 32 consecutive bins, one bin per lane (conflict-free shared-memory reads), the peak predicate
+    // of a chunk kept as a 32-bit ballot; pass 2: every thread owns a contiguous range of chunks, a block scan of the
+    // popcounts gives the position of each peak in linear-index order.
+    uint32_t* s_ballot = reinterpret_cast<uint32_t*>(s_rc + NR);     // [bins / 32]
+    const uint32_t chunks = bins / 32u;                              // bins % 32 == 0 (n_vtx_phi % 4 == 0, n_vtx_r % 8 == 0)
+    for (uint32_t q = warp; q < chunks; q += kVtxThreads / 32) {
+        const uint32_t bb = q * 32u + (uint32_t)lane;
+        const uint32_t c = vcount(acc, bb);
+        const bool pk1 = c >= p.n_min && vtx_is_peak(acc, NPV, NR, (int)(bb / (uint32_t)NR), (int)(bb % (uint32_t)NR), c);
+        const uint32_t bal = __ballot_sync(0xffffffffu, pk1);
+        if (lane == 0) s_ballot[q] = bal;
     }
+    __syncthreads();
+    const uint32_t per = (chunks + kVtxThreads - 1) / kVtxThreads;
+    const uint32_t q_lo = min((uint32_t)tid * per, chunks), q_hi = min(q_lo + per, chunks);
+    uint32_t mine = 0;
+    for (uint32_t q = q_lo; q < q_hi; ++q) mine += (uint32_t)__popc(s_ballot[q]);
     uint32_t incl = mine;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -154,17 +170,17 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
     __syncthreads();
     uint32_t pos = s_warp[warp] + incl - mine;
     hough_vertex* out = p.vertices + (size_t)e * p.max_vertices;
-    if (mine > 0 && pos < p.max_vertices) {
-        for (uint32_t b = b_lo; b < b_hi && pos < p.max_vertices; ++b) {
-            const uint32_t c = vcount(acc, b);
-            const int iv = (int)(b / (uint32_t)NR), ir = (int)(b % (uint32_t)NR);
-            if (c >= p.n_min && vtx_is_peak(acc, NPV, NR, iv, ir, c)) {
-                hough_vertex vx;
-                vx.r = p.rc[ir];
-                vx.phi = (float)(((double)iv + 0.5) * p.dphi_v);
-                vx.n_tracks = c; vx.lin = b;
-                out[pos++] = vx;
-            }
+    for (uint32_t q = q_lo; q < q_hi && pos < p.max_vertices; ++q) {
+        uint32_t word = s_ballot[q];
+        while (word && pos < p.max_vertices) {
+            const uint32_t bb = q * 32u + (uint32_t)(__ffs(word) - 1);
+            word &= word - 1;
+            const int iv = (int)(bb / (uint32_t)NR), ir = (int)(bb % (uint32_t)NR);
+            hough_vertex vx;
+            vx.r = s_rc[ir];
+            vx.phi = (float)(((double)iv + 0.5) * p.dphi_v);
+            vx.n_tracks = vcount(acc, bb); vx.lin = bb;
+            out[pos++] = vx;
         }
     }
     if (tid == 0) { p.n_vertices[e] = s_total; p.flag[e] = s_total > 0u ? 1 : 0; }
@@ -187,7 +203,8 @@ cudaError_t launch_vertices(hough_ctx* c, uint32_t n_events, const hough_peak* d
     p.n_vphi = (int)c->cfg.n_vtx_phi; p.n_vr = (int)c->cfg.n_vtx_r;
     p.d0_cut = d0_cut; p.n_min = n_min;
     p.dphi_v = 6.283185307179586476925286766559 / (double)c->cfg.n_vtx_phi;
-    const size_t smem = (size_t)c->cfg.n_vtx_phi * c->cfg.n_vtx_r * 2;
+    const size_t bins = (size_t)c->cfg.n_vtx_phi * c->cfg.n_vtx_r;
+    const size_t smem = bins * 2 + (2 * (size_t)c->cfg.n_vtx_phi + c->cfg.n_vtx_r) * 4 + bins / 32 * 4;
     cudaError_t err = cudaFuncSetAttribute(vertex_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
     vertex_kernel<<<n_events, kVtxThreads, smem, st>>>(p);
