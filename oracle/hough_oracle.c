@@ -504,3 +504,110 @@ uint32_t oracle_vertices(const oracle_grid *g, const oracle_vgrid *v, const orac
     free(count); free(mask); free(d0); free(s0); free(c0); free(kap); free(pk);
     return (uint32_t)total;
 }
+
+/* ================================================================================================ */
+/* O-2h / O-2f: physics-quality voting variants (the paper's future work is       */
+/* "efficiency and purity improvements").  DESIGN.md readings R40-R42.                 */
+/*   ORACLE_VOTE_HEMI  forward-hemisphere cut: a (hit, column) pair votes only if                    */
+/*                     ch = fl(fl(cp*c0) + fl(sp*s0)) = cos(phi - phi0c) > 0 -- removes the mirror    */
+/*                     solutions (phi0 + pi, -d0, -kappa) of reading R5 and halves the votes.         */
+/*   ORACLE_VOTE_FILL  kappa-range filling: instead of one vote at the column CENTRE (R4), the O-2   */
+/*                     chain is evaluated at the two phi0 EDGES of the column, phi0e(j) = j 2pi/NPHI  */
+/*                     (tables of NPHI edges, each (float)cos / (float)sin of the double angle; edge  */
+/*                     NPHI is edge 0), giving ua, ub; the hit votes once in EVERY kappa bin between  */
+/*                     floor(min) and floor(max), clipped to the axis -- the curve of a hit becomes a  */
+/*                     connected band, so tracks that are not aligned with a bin centre collect all   */
+/*                     their layers in one bin.  No vote if either u is NaN or both lie on the same   */
+/*                     side outside the axis.  The hemisphere test (if set) stays at the centre.      */
+/* ================================================================================================ */
+
+enum { ORACLE_VOTE_HEMI = 1u, ORACLE_VOTE_FILL = 2u };
+
+/* u of O-2 (the kappa-bin coordinate before the range test) for one (hit, d0 bin, direction (c0, s0)) */
+static float vote_u(int mode3d, float r, float r2, float sp, float cp, float c0, float s0, float d0c, float two_d0,
+                    float d0sq, float kmax, float inv_dk)
+{
+    float m1 = sp * c0;
+    float m2 = cp * s0;
+    float s = m1 - m2;
+    float kappa;
+    if (!mode3d) {
+        float two_s = 2.0f * s;
+        kappa = two_s / r;
+    } else {
+        float rs = r * s;
+        float t = rs + d0c;
+        float num = 2.0f * t;
+        float a = two_d0 * rs;
+        float b = r2 + a;
+        float den = b + d0sq;
+        kappa = num / den;
+    }
+    float v = kappa + kmax;
+    float u = v * inv_dk;
+    return u;
+}
+
+int64_t oracle_vote_variant(const oracle_grid *g, uint32_t flags, uint64_t n_hits, const float *r, const float *phi,
+                            const uint8_t *layer, uint16_t *count, uint16_t *mask)
+{
+    const int mode3d = g->n_d0 > 1;
+    const float kmax = g->kappa_max;
+    const float inv_dk = inv_dkappa(g);
+    const float nk_f = (float)g->n_kappa;
+    const int NK = (int)g->n_kappa;
+    int64_t votes = 0;
+    float *c0 = (float *)malloc(sizeof(float) * g->n_phi0), *s0 = (float *)malloc(sizeof(float) * g->n_phi0);
+    float *ce = (float *)malloc(sizeof(float) * g->n_phi0), *se = (float *)malloc(sizeof(float) * g->n_phi0);
+    float *d0c = (float *)malloc(sizeof(float) * g->n_d0);
+    float inv_unused;
+    oracle_tables(g, c0, s0, d0c, &inv_unused);
+    for (uint32_t j = 0; j < g->n_phi0; ++j) {                 /* column edges: phi0e(j) = j * 2pi / NPHI */
+        const double a = (double)j * (2.0 * M_PI / (double)g->n_phi0);
+        ce[j] = (float)cos(a);
+        se[j] = (float)sin(a);
+    }
+    for (uint64_t h = 0; h < n_hits; ++h) {
+        if (layer[h] >= g->n_layers) continue;
+        const float sp = hit_sin(phi[h]);
+        const float cp = hit_cos(phi[h]);
+        const float rr = r[h];
+        const float r2 = rr * rr;
+        const uint16_t bit = (uint16_t)(1u << layer[h]);
+        for (uint32_t ip = 0; ip < g->n_phi0; ++ip) {
+            if (flags & ORACLE_VOTE_HEMI) {
+                float h1 = cp * c0[ip];
+                float h2 = sp * s0[ip];
+                float ch = h1 + h2;                            /* cos(phi - phi0c) */
+                if (!(ch > 0.0f)) continue;
+            }
+            const uint32_t jp = (ip + 1 == g->n_phi0) ? 0 : ip + 1;
+            for (uint32_t id = 0; id < g->n_d0; ++id) {
+                const float two_d0 = 2.0f * d0c[id];
+                const float d0sq = d0c[id] * d0c[id];
+                int klo, khi;
+                if (flags & ORACLE_VOTE_FILL) {
+                    const float ua = vote_u(mode3d, rr, r2, sp, cp, ce[ip], se[ip], d0c[id], two_d0, d0sq, kmax, inv_dk);
+                    const float ub = vote_u(mode3d, rr, r2, sp, cp, ce[jp], se[jp], d0c[id], two_d0, d0sq, kmax, inv_dk);
+                    if (!(ua == ua) || !(ub == ub)) continue;  /* NaN at an edge: no vote */
+                    const float lo = (ua < ub) ? ua : ub, hi = (ua < ub) ? ub : ua;
+                    if (hi < 0.0f || lo >= nk_f) continue;     /* the whole band lies outside the axis */
+                    klo = (lo < 0.0f) ? 0 : (int)lo;
+                    khi = (hi >= nk_f) ? NK - 1 : (int)hi;
+                } else {
+                    const float u = vote_u(mode3d, rr, r2, sp, cp, c0[ip], s0[ip], d0c[id], two_d0, d0sq, kmax, inv_dk);
+                    if (!(u >= 0.0f && u < nk_f)) continue;
+                    klo = khi = (int)u;
+                }
+                for (int k = klo; k <= khi; ++k) {
+                    size_t b = ((size_t)id * g->n_phi0 + ip) * g->n_kappa + (size_t)k;
+                    count[b] = (uint16_t)(count[b] + 1);
+                    mask[b] |= bit;
+                    ++votes;
+                }
+            }
+        }
+    }
+    free(c0); free(s0); free(ce); free(se); free(d0c);
+    return votes;
+}

@@ -72,6 +72,8 @@ def _load():
         lib.oracle_jets.argtypes = [C.POINTER(_Grid), p, C.c_uint32, C.c_float, C.c_float, C.c_uint32,
                                     C.c_uint32, p, p, p]
         lib.oracle_jets.restype = C.c_uint32
+        lib.oracle_vote_variant.argtypes = [C.POINTER(_Grid), C.c_uint32, C.c_uint64, p, p, p, p, p]
+        lib.oracle_vote_variant.restype = C.c_int64
         lib.oracle_angle_bin.argtypes = [C.POINTER(_VGrid), C.c_float, C.c_float]
         lib.oracle_angle_bin.restype = C.c_uint32
         lib.oracle_vertex_vote.argtypes = [C.POINTER(_VGrid), C.c_uint32, p, p, p, p, C.c_float, p]
@@ -190,6 +192,19 @@ def vote(g: Grid, r, phi, layer, id_range: Optional[Tuple[int, int]] = None,
     cg = g.c()
     n = _load().oracle_vote(C.byref(cg), r.size, _ptr(r), _ptr(phi), _ptr(layer), id_lo, id_hi, ip_lo, ip_hi,
                             _ptr(count), _ptr(mask))
+    return count, mask, int(n)
+
+
+VOTE_HEMI, VOTE_FILL = 1, 2
+
+
+def vote_variant(g: Grid, flags: int, r, phi, layer):
+    """O-2 with the physics-quality variants (VOTE_HEMI forward-hemisphere cut, VOTE_FILL kappa-range filling between
+    the phi0 edges of a column) for ONE event: (count, mask) uint16 [ND, NPHI, NK], votes.  flags = 0 is O-2 itself."""
+    r, phi, layer = _hits(r, phi, layer)
+    count = np.zeros(g.shape, np.uint16); mask = np.zeros(g.shape, np.uint16)
+    cg = g.c()
+    n = _load().oracle_vote_variant(C.byref(cg), flags, r.size, _ptr(r), _ptr(phi), _ptr(layer), _ptr(count), _ptr(mask))
     return count, mask, int(n)
 
 

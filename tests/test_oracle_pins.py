@@ -811,3 +811,93 @@ def test_p17_vertices_reuse_the_peak_finder_and_drop_the_interaction_point():
         assert tot == len(ref) and [int(x) for x in vt["lin"]] == [l for l, _ in ref][:4096]
         assert [int(x) for x in vt["n_tracks"]] == [c for _, c in ref][:4096]
         assert np.allclose(vt["r"], rc[vt["lin"] % 128], rtol=1e-6) and np.allclose(vt["phi"], pc[vt["lin"] // 128], rtol=1e-6)
+
+
+# ----------------------------------------------------------------------------------------------
+# P18-P20: physics-quality voting variants (forward-hemisphere cut, kappa-range filling), SURVEY 8(f)-3
+# ----------------------------------------------------------------------------------------------
+
+def test_p18_variant_flags_zero_is_the_plain_vote_and_hemisphere_drops_the_mirror():
+    g = O.Grid(128, 64, 8, KMAX, -40.0, 40.0)
+    w = W.scaled(W.config(2), n_d0=8, n_phi0=128, n_kappa=64, d0_min=-40.0, d0_max=40.0)
+    r, phi, layer, _ = W.generate_event(w, 3)
+    c0, m0, v0 = O.vote(g, r, phi, layer)
+    c1, m1, v1 = O.vote_variant(g, 0, r, phi, layer)
+    assert np.array_equal(c0, c1) and np.array_equal(m0, m1) and v0 == v1
+    # hemisphere: votes = in-range triples with cos(phi - phi0c) > 0, counted independently in fp64
+    ch, mh, vh = O.vote_variant(g, O.VOTE_HEMI, r, phi, layer)
+    d0c, phi0c, _, _ = bin_centres(g)
+    keep = near = 0
+    for rr, ph in zip(r.astype(np.float64), phi.astype(np.float64)):
+        for d in d0c:
+            u = u_double(g, rr, ph, d, phi0c)
+            cosd = np.cos(ph - phi0c)
+            inr = (u >= 0) & (u < g.n_kappa)
+            keep += int((inr & (cosd > 0)).sum())
+            near += int((inr & (np.abs(cosd) < 1e-6)).sum()) + int((np.abs(u - np.round(u)) < 2e-3)[cosd > 0].sum())
+    assert abs(vh - keep) <= near + 2 and vh < 0.6 * v0
+    assert np.all(ch <= c0) and np.all((mh & ~m0) == 0)
+    # a bin-centred noiseless track keeps its peak and loses its mirror image (R5)
+    ip, ik, idd = 20, 40, 5
+    kap = -float(np.float32(KMAX)) + (ik + 0.5) * (2 * float(np.float32(KMAX)) / 64)
+    rad = np.float64(W.TRACKER_A)
+    # exact layer crossings by the generator's own forward model
+    d0t, phi0t = np.array([d0c[idd]]), np.array([phi0c[ip]])
+    from paper_1309_6275_b200.workloads import _displaced_hits
+    px, py = d0t * np.sin(phi0t), -d0t * np.cos(phi0t)
+    hr, hp, hl = _displaced_hits(px, py, phi0t, np.array([kap]), rad, np.array([abs(d0t[0])]))
+    cnt, msk, _ = O.vote_variant(g, O.VOTE_HEMI, hr.astype(np.float32), np.mod(hp, TWO_PI).astype(np.float32), hl.astype(np.uint8))
+    cntp, _, _ = O.vote(g, hr.astype(np.float32), np.mod(hp, TWO_PI).astype(np.float32), hl.astype(np.uint8))
+    assert cnt[idd, ip, ik] == hr.size == cntp[idd, ip, ik]
+    mirror = (8 - 1 - idd, (ip + 64) % 128, 64 - 1 - ik)
+    assert cntp[mirror] == hr.size and cnt[mirror] == 0
+
+
+def test_p19_filling_lets_unaligned_tracks_collect_all_their_layers():
+    """R4's gaps: with one vote at the column centre a track whose phi0 is not on a bin centre spreads its layers over
+    neighbouring kappa bins; with the kappa range between the column edges filled, the bin that contains its true
+    (phi0, kappa) collects every layer (PAPER.md:169 'efficiency ... improvements')."""
+    g = O.Grid(512, 256)
+    rng = np.random.default_rng(19)
+    rad = np.float64(W.TRACKER_A)
+    full_plain = full_fill = 0
+    n = 40
+    for _ in range(n):
+        phi0 = rng.uniform(0, TWO_PI); kap = rng.choice([-1.0, 1.0]) * KMAX / rng.uniform(1.2, 20.0)
+        ph = np.mod(phi0 + np.arcsin(0.5 * kap * rad), TWO_PI).astype(np.float32)
+        r = rad.astype(np.float32); lay = np.arange(8, dtype=np.uint8)
+        ip = int(phi0 / (TWO_PI / 512)); ik = int((kap + float(np.float32(KMAX))) / (2 * float(np.float32(KMAX)) / 256))
+        cp_, _, _ = O.vote(g, r, ph, lay)
+        cf, mf, _ = O.vote_variant(g, O.VOTE_FILL, r, ph, lay)
+        full_plain += int(cp_[0, ip, ik] == 8)
+        full_fill += int(cf[0, ip, ik] == 8 and mf[0, ip, ik] == 0xFF)
+    assert full_fill == n and full_plain < n // 2
+
+
+def test_p20_filled_bands_match_an_fp64_evaluation_at_the_column_edges():
+    g = O.Grid(64, 48, 6, KMAX, -30.0, 30.0)
+    rng = np.random.default_rng(20)
+    n = 60
+    r = rng.choice(np.float64(W.TRACKER_A), n).astype(np.float32); phi = rng.uniform(0, TWO_PI, n).astype(np.float32)
+    lay = rng.integers(0, 8, n).astype(np.uint8)
+    cf, mf, vf = O.vote_variant(g, O.VOTE_FILL | O.VOTE_HEMI, r, phi, lay)
+    d0c, phi0c, _, _ = bin_centres(g)
+    edges = np.arange(65) * (TWO_PI / 64)
+    ref = np.zeros(g.shape, np.int64); fuzzy = np.zeros(g.shape, bool)
+    for rr, ph, l in zip(r.astype(np.float64), phi.astype(np.float64), lay):
+        for idd, d in enumerate(d0c):
+            ua = u_double(g, rr, ph, d, edges[:-1]); ub = u_double(g, rr, ph, d, edges[1:])
+            cosc = np.cos(ph - phi0c)
+            for ip in range(64):
+                if abs(cosc[ip]) < 1e-6: fuzzy[idd, ip, :] = True
+                if cosc[ip] <= 0: continue
+                lo, hi = min(ua[ip], ub[ip]), max(ua[ip], ub[ip])
+                if not np.isfinite(lo) or not np.isfinite(hi) or hi < 0 or lo >= 48: continue
+                klo, khi = max(int(np.floor(lo)), 0), min(int(np.floor(hi)), 47)
+                ref[idd, ip, klo:khi + 1] += 1
+                for x in (lo, hi):                               # an edge value within 2e-3 of a bin boundary may fall either side
+                    if abs(x - round(x)) < 2e-3: fuzzy[idd, ip, max(int(round(x)) - 1, 0):int(round(x)) + 1] = True
+    ok = ~fuzzy
+    assert ok.sum() > 0.9 * ok.size
+    assert np.array_equal(cf.astype(np.int64)[ok], ref[ok])
+    assert vf > 2 * O.vote_variant(g, O.VOTE_HEMI, r, phi, lay)[2]
