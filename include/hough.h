@@ -55,7 +55,17 @@ typedef struct {
                                       n_vtx_phi * n_vtx_r * 2 bytes must fit in shared memory (<= 200 KB)            */
     float    vtx_r_min, vtx_r_max; /* mm; vtx_r_min = radius inside which vertices are dropped (beam pipe, 30 mm)     */
     uint32_t max_vertices_per_event;
+    uint32_t vote_flags;           /* physics-quality voting variants (O-2h / O-2f), accumulator
+                                      path only: HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL; 0 = the normative one-vote-per-column-
+                                      centre rule of north_star.  hough_vote_peaks / hough_trigger_host* return
+                                      HOUGH_EUNSUPPORTED when it is not 0                                             */
 } hough_config;
+
+enum {
+    HOUGH_VOTE_HEMI = 1u,   /* forward-hemisphere cut: a (hit, column) votes only if cos(phi - phi0c) > 0 (no mirror peaks) */
+    HOUGH_VOTE_FILL = 2u    /* kappa-range filling: one vote in every kappa bin between the values at the two phi0 edges
+                               of the column, so a hit's curve is a connected band ("efficiency ... improvements") */
+};
 
 typedef struct { uint32_t lin; uint16_t count; uint16_t mask; } hough_peak;                     /*  8 B */
 typedef struct { float pt, phi0, d0; int32_t q; int32_t jet; } hough_track;                     /* 20 B */

@@ -41,6 +41,7 @@ void free_all(hough_ctx* c)
     cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_cand); cudaFree(c->d_cand_n); cudaFree(c->d_sortkeys);
+    cudaFree(c->d_ce); cudaFree(c->d_se);
     cudaFree(c->d_kc); cudaFree(c->d_vex); cudaFree(c->d_vey); cudaFree(c->d_vrc);
     cudaFree(c->d_hp_vertices); cudaFree(c->d_hp_nvtx); cudaFree(c->d_hp_vflag);
     cudaFree(c->d_hp_count); cudaFree(c->d_hp_mask); cudaFree(c->d_hp_off); cudaFree(c->d_hp_r);
@@ -81,6 +82,7 @@ bool config_ok(const hough_config* g)
     if (g->max_peaks_per_event < 1 || g->max_jets_per_event < 1) return false;
     if (g->host_chunk_events > g->max_events) return false;
     if (g->max_candidates_per_event > (1u << 24)) return false;
+    if (g->vote_flags & ~(uint32_t)(HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL)) return false;
     if (g->n_vtx_phi != 0) {                                   // vertex grid of the second transform
         if (g->n_vtx_phi < 8 || g->n_vtx_phi % 4 != 0 || g->n_vtx_r < 8 || g->n_vtx_r % 8 != 0) return false;
         if ((uint64_t)g->n_vtx_phi * g->n_vtx_r * 2 > 200u * 1024u) return false;
@@ -158,7 +160,12 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
                               ((double)ir + 0.5) * (((double)cfg->vtx_r_max - (double)cfg->vtx_r_min) / (double)cfg->n_vtx_r));
     }
     // mirror tiles need tables that are antisymmetric bit for bit: c0[ip + N/2] == -c0[ip], s0 likewise, d0c[ND-1-id] == -d0c[id]
-    bool mirror_ok = NP % 2 == 0 && getenv("HOUGH_NO_MIRROR") == nullptr;
+    std::vector<float> ce(NP), se(NP);                         // column edges (voting variant FILL)
+    for (uint32_t j = 0; j < NP; ++j) {
+        const double a = (double)j * (2.0 * pi / (double)NP);
+        ce[j] = (float)cos(a); se[j] = (float)sin(a);
+    }
+    bool mirror_ok = NP % 2 == 0 && getenv("HOUGH_NO_MIRROR") == nullptr && cfg->vote_flags == 0;
     for (uint32_t ip = 0; mirror_ok && ip < NP / 2; ++ip)
         mirror_ok = c0[ip + NP / 2] == -c0[ip] && s0[ip + NP / 2] == -s0[ip];
     for (uint32_t id = 0; mirror_ok && id < ND; ++id) mirror_ok = d0c[ND - 1 - id] == -d0c[id];
@@ -179,6 +186,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_c0, NP)); A(dev_alloc(&c->d_s0, NP));
     A(dev_alloc(&c->d_d0c, ND)); A(dev_alloc(&c->d_two_d0, ND)); A(dev_alloc(&c->d_d0sq, ND));
     A(dev_alloc(&c->d_kc, NK));
+    A(dev_alloc(&c->d_ce, NP)); A(dev_alloc(&c->d_se, NP));
     A(dev_alloc(&c->d_vex, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vey, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vrc, cfg->n_vtx_r));
     A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_rec_u, cfg->max_hits)); A(dev_alloc(&c->d_key, cfg->max_hits));
     A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
@@ -235,6 +243,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemcpy(c->d_d0sq, d0sq.data(), ND * 4, cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_layer_r, lr, sizeof(lr), cudaMemcpyHostToDevice));
     A(cudaMemcpy(c->d_kc, kc.data(), NK * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_ce, ce.data(), NP * 4, cudaMemcpyHostToDevice));
+    A(cudaMemcpy(c->d_se, se.data(), NP * 4, cudaMemcpyHostToDevice));
     if (cfg->n_vtx_phi) {
         A(cudaMemcpy(c->d_vex, vex.data(), vex.size() * 4, cudaMemcpyHostToDevice));
         A(cudaMemcpy(c->d_vey, vey.data(), vey.size() * 4, cudaMemcpyHostToDevice));
@@ -304,6 +314,7 @@ int hough_vote_peaks(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_of
     if (n_hits_total > 0 && (!d_r || !d_phi || !d_layer)) return HOUGH_EINVAL;
     if (n_events > ctx->cfg.max_events || n_events > ctx->fused_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
     if (l_min < 1 || l_min > ctx->cfg.n_layers) return HOUGH_EINVAL;
+    if (ctx->cfg.vote_flags != 0) return HOUGH_EUNSUPPORTED;      // voting variants: accumulator path only
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     if (n_events == 0) return HOUGH_OK;
@@ -366,6 +377,7 @@ int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_
 {
     if (!ctx || !h_hit_offsets || !h_n_peaks || !h_n_jets || !h_flag) return HOUGH_EINVAL;
     if (ctx->cfg.host_chunk_events == 0) return HOUGH_EINVAL;
+    if (ctx->cfg.vote_flags != 0) return HOUGH_EUNSUPPORTED;      // voting variants: accumulator path only
     if (n_hits_total > 0 && (!h_r || !h_phi || !h_layer)) return HOUGH_EINVAL;
     if (n_events > ctx->cfg.max_events || n_hits_total > ctx->cfg.max_hits) return HOUGH_EINVAL;
     if (l_min < 1 || l_min > ctx->cfg.n_layers || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm))

@@ -54,6 +54,7 @@ struct hough_ctx {
     float* d_c0; float* d_s0;                 // [NPHI]
     float* d_d0c; float* d_two_d0; float* d_d0sq;   // [ND]
     float kmax, inv_dk, nk_f;
+    float* d_ce; float* d_se;                 // [NPHI] (cos, sin) of the phi0 column edges j * 2pi / NPHI (voting variant FILL)
     float* d_kc;                              // [NK] kappa bin centres, fp32 rounded once from double (O-6)
     float* d_vex; float* d_vey;               // [n_vtx_phi] phi_v bin-edge directions (cos, sin)(k * 2pi / n_vtx_phi)
     float* d_vrc;                             // [n_vtx_r] R_v bin centres

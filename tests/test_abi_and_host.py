@@ -38,9 +38,9 @@ def test_strerror_and_argument_validation_without_gpu():
     assert B.strerror(0) == "ok" and "invalid" in B.strerror(-1)
     # a bad config is rejected before any CUDA call; null pointers likewise
     ctx = C.c_void_p()
-    bad = B.HoughConfig(512, 250, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0)       # n_kappa % 8 != 0
+    bad = B.HoughConfig(512, 250, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0)       # n_kappa % 8 != 0
     assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
-    bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0)     # n_layers > 16
+    bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0)     # n_layers > 16
     assert lib.hough_create(C.byref(bad2), C.byref(ctx)) == -1
     assert lib.hough_create(None, C.byref(ctx)) == -1
     assert lib.hough_destroy(None) == -1
@@ -57,7 +57,8 @@ def test_config_struct_layout_matches_header():
     int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(hough_config), offsetof(hough_config, max_hits),
         offsetof(hough_config, host_chunk_events), sizeof(hough_peak), sizeof(hough_track), sizeof(hough_jet),
         offsetof(hough_config, max_events), offsetof(hough_config, max_candidates_per_event));
-        printf("%zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex));
+        printf("%zu %zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex),
+               offsetof(hough_config, vote_flags));
         return 0; }'''
     exe = os.path.join(ROOT, "_work", "layout_probe") if os.path.isdir(os.path.join(ROOT, "_work")) else "/tmp/layout_probe"
     exe = "/tmp/hough_layout_probe"
@@ -67,7 +68,7 @@ def test_config_struct_layout_matches_header():
     assert vals[1] == B.HoughConfig.max_hits.offset and vals[2] == B.HoughConfig.host_chunk_events.offset
     assert vals[6] == B.HoughConfig.max_events.offset and vals[7] == B.HoughConfig.max_candidates_per_event.offset
     assert vals[8] == B.HoughConfig.vtx_r_min.offset and vals[9] == B.HoughConfig.max_vertices_per_event.offset
-    assert vals[10] == B.VERTEX_DTYPE.itemsize == 16
+    assert vals[10] == B.VERTEX_DTYPE.itemsize == 16 and vals[11] == B.HoughConfig.vote_flags.offset
     assert vals[3] == B.PEAK_DTYPE.itemsize == 8 and vals[4] == B.TRACK_DTYPE.itemsize == 20
     assert vals[5] == B.JET_DTYPE.itemsize == 20
 
@@ -80,11 +81,15 @@ def test_packed_sweep_keeps_every_rounding_of_o2():
     from paper_1309_6275_b200 import build
     lib = build.build()
     sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
-    kernels = [b for b in sass.split("Function : ")[1:] if "vote_kernelILb1E" in b.split("\n")[0]]
+    # vote_kernel<MODE3D, KL, FUSED, MIRROR, VARIANT>: the packed 3D kernels (the scalar voting-variant kernels are left out)
+    kernels = []
+    for body in sass.split("Function : ")[1:]:
+        m = re.search(r"vote_kernelILb(\d)ELi(\d)ELb(\d)ELb(\d)ELb(\d)EEEv", body.split("\n")[0])
+        if m and m.group(1) == "1" and m.group(5) == "0":
+            kernels.append((m.group(4) == "1", body))
     assert len(kernels) == 8                                     # KL = 1, 2, 4 x {planes, fused} + the two mirror kernels
     n_mirror = 0
-    for body in kernels:
-        mirror = re.search(r"Lb([01])EEEvNS", body.split("\n")[0]).group(1) == "1"     # ..., bool MIRROR>
+    for mirror, body in kernels:
         n_rm = len(re.findall(r"\bFADD2\.RM\b", body))
         n_add = len(re.findall(r"\bFADD2 ", body))
         n_mul = len(re.findall(r"\bFMUL2 ", body))
