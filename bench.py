@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- whole hot path (vote -> peaks -> tracks -> jets) on synthetic trigger batches, one JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3|C2|C1|P4] [--events E]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C4|C3|C2|C1|P4|F8|F9|F10] [--events E]
                   [--path fused|planes] [--impl ours|reference] [--tracks N]
 
 A "step" is one pass of the whole hot path over one batch (BASELINE.json configs[4] by default: 4,096 events,
@@ -516,6 +516,127 @@ def run_p4(args):
     print(json.dumps(line))
 
 
+def match_vertices(found_r, found_phi, true_r, true_phi, tol_mm: float):
+    """Truth matching of the efficiency studies: a simulated jet counts as identified if a found vertex lies within
+    tol_mm of its vertex in the transverse plane (PAPER.md:137 'fraction of simulated jets successfully identified').
+    Returns (true vertices matched, found vertices that match no true vertex)."""
+    fx, fy = found_r * np.cos(found_phi), found_r * np.sin(found_phi)
+    tx, ty = true_r * np.cos(true_phi), true_r * np.sin(true_phi)
+    if tx.size == 0 or fx.size == 0:
+        return 0, int(fx.size)
+    d = np.hypot(fx[:, None] - tx[None, :], fy[:, None] - ty[None, :])
+    return int((d.min(axis=0) <= tol_mm).sum()), int((d.min(axis=1) > tol_mm).sum())
+
+
+def efficiency_point(w, batch, flags: int, steps: int, warmup: int, tol_mm: float):
+    """One point of an efficiency study: the whole chain on the GPU for the batch, then truth matching on the host."""
+    import torch
+    from paper_1309_6275_b200 import binding as B
+    E = batch.n_events
+    stream = torch.cuda.current_stream()
+    chunk = max(1, min(E, int(4e9 // (4 * w.bins_per_event))))
+    off, r, phi, layer = B.upload_batch(batch)
+    offs = batch.hit_offsets.astype(np.int64)
+    hits_per_chunk = max(int(offs[min(c + chunk, E)] - offs[c]) for c in range(0, E, chunk))
+    h = B.Hough.for_workload(w, max_events=chunk, max_hits=hits_per_chunk, vgrid=w.vgrid, max_vertices=w.max_vertices,
+                             vote_flags=flags)
+    count, mask = h.alloc_planes(chunk)
+    out = h.alloc_outputs(E)
+
+    def step():
+        for e0 in range(0, E, chunk):
+            ne = min(chunk, E - e0)
+            hb, he = int(offs[e0]), int(offs[e0 + ne])
+            h.hough_vote(ne, off[e0:e0 + ne + 1], he - hb, r[hb:he], phi[hb:he], layer[hb:he], count, mask, stream)
+            h.hough_peaks(ne, count, mask, w.l_min, out["peaks"][e0:], out["n_peaks"][e0:], stream)
+            h.hough_jets(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.cone_rad, w.d0_cut_mm, w.n_displaced_min,
+                         out["tracks"][e0:], out["jets"][e0:], out["n_jets"][e0:], out["flag"][e0:], stream)
+            h.hough_vertices(ne, out["peaks"][e0:], out["n_peaks"][e0:], w.d0_cut_mm, w.vtx_n_min, out["vertices"][e0:],
+                             out["n_vertices"][e0:], out["vtx_flag"][e0:], None, stream)
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    l0 = h.hough_launch_count()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for _ in range(steps):
+        step()
+    b.record(stream)
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / steps
+    nv = out["n_vertices"].cpu().numpy()
+    vt = B.records(out["vertices"], B.VERTEX_DTYPE)
+    npk = out["n_peaks"].cpu().numpy().astype(np.int64)
+    found = fake = n_true = 0
+    for e in range(E):
+        k = min(int(nv[e]), w.max_vertices)
+        t = batch.truth[e]
+        tr = t.get("vertex_r", np.zeros(0)); tp = t.get("vertex_phi", np.zeros(0))
+        m, f = match_vertices(vt[e, :k]["r"].astype(np.float64), vt[e, :k]["phi"].astype(np.float64), tr, tp, tol_mm)
+        found += m; fake += f; n_true += int(tr.size)
+    res = {"efficiency": found / max(1, n_true), "jets_found": found, "unmatched_vertices_per_event": fake / E,
+           "peaks_per_event": float(npk.mean()), "peak_list_overflows": int((npk > w.max_peaks).sum()),
+           "ms_per_event": ms / E, "status_bits": int(h.hough_status()), "launches": int(h.hough_launch_count() - l0)}
+    h.close()
+    del count, mask, out
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_efficiency(args):
+    """--workload F8 | F9 | F10: the SHAPE of the paper's efficiency studies (Figs 8-10) on synthetic
+    events of its toy detector: efficiency of displaced-jet detection against tracks per jet (F8), jets per event (F9),
+    and jets per event among 3,000 tracks (F10).  Whole chain on the GPU through the C-ABI: hough_vote with the
+    physics-quality voting variants (forward-hemisphere cut + kappa-range filling) -> hough_peaks ->
+    hough_jets -> hough_vertices (second Hough transform, vertices inside the beam pipe dropped); the plain one-vote-per-
+    column-centre vote is run next to it.  Only the truth matching happens on the host."""
+    import torch
+    from paper_1309_6275_b200 import binding as B
+    from paper_1309_6275_b200 import workloads as W
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1 or args.gpus != 1:
+        raise SystemExit("bench.py --workload F8/F9/F10 is a single-GPU study")
+    torch.cuda.set_device(0)
+    kind = args.workload
+    xs = {"F8": [2, 4, 6, 8, 10, 12, 15, 20], "F9": [1, 2, 3, 4, 6, 8, 10], "F10": [1, 2, 4, 6, 8, 10]}[kind]
+    if args.tracks:
+        xs = [args.tracks]
+    E = args.events or (32 if kind == "F10" else 64)
+    tol_mm = 10.0
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    wall0 = time.time()
+    curve, last_ms, launches = [], None, 0
+    for x in xs:
+        w = W.paper_efficiency(kind, x, E)
+        batch = W.generate(w, keep_truth=True)
+        d = {"x": x, "hits_per_event": batch.n_hits // E, "jets_simulated": int(sum(t["n_vertices"] for t in batch.truth))}
+        for label, flags in (("variants", w.vote_flags), ("plain", 0)):
+            d[label] = efficiency_point(w, batch, flags, args.steps, max(1, args.warmup), tol_mm)
+            if label == "variants":
+                last_ms, launches, last = d[label]["ms_per_event"] * E, d[label].pop("launches"), (w, batch)
+            else:
+                d[label].pop("launches")
+        curve.append(d)
+    clocks = sampler.stop(wall0, time.time())
+    w, batch = last
+    line = {"metric": "events_per_sec", "value": E / (last_ms * 1e-3), "unit": "events/s", "n_gpus": 1, "steps": args.steps,
+            "warmup": max(1, args.warmup), "ms_per_step": last_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "path": "planes (hough_vote with vote_flags %d)" % w.vote_flags,
+                       "events_per_gpu": E, "hits": batch.n_hits, "grid": [w.n_d0, w.n_phi0, w.n_kappa], "l_min": w.l_min,
+                       "vertex_grid": list(w.vgrid), "vtx_n_min": w.vtx_n_min, "d0_cut_mm": w.d0_cut_mm, "match_tol_mm": tol_mm,
+                       "detector": "PAPER.md:97-99: beam pipe 30 mm, 10 layers evenly spaced to 1100 mm, 0.4 mm resolution",
+                       "l2": "planes (67 MB per event, rewritten every launch) are larger than L2",
+                       "note": "shape of the paper's efficiency studies (PAPER.md:137-151); its figures are not readable, "
+                               "so there is no number to compare with"},
+            "study": {"F8": "efficiency vs tracks per displaced jet (PAPER.md:137, Fig. 8)",
+                      "F9": "efficiency vs displaced jets per event, 10 tracks each (PAPER.md:145, Fig. 9)",
+                      "F10": "efficiency vs displaced jets per event among 3000 tracks (PAPER.md:147, Fig. 10)"}[kind],
+            "curve_efficiency": curve, "clocks": clocks, "gpu_launches": int(launches)}
+    print(json.dumps(line))
+
+
 def run_ours(args):
     import torch
     from paper_1309_6275_b200 import binding as B
@@ -704,8 +825,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "P4"])
-    ap.add_argument("--tracks", type=int, default=0, help="P4 only: one point of the curve (0 = 100, 300, 1000, 3000)")
+    ap.add_argument("--workload", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "P4", "F8", "F9", "F10"])
+    ap.add_argument("--tracks", type=int, default=0, help="P4 / F8 / F9 / F10: one point of the curve (0 = all of them)")
     ap.add_argument("--path", default="fused", choices=["fused", "planes"])
     ap.add_argument("--events", type=int, default=0, help="override the number of events per GPU (0 = the config's)")
     ap.add_argument("--chunk", type=int, default=0, help="events per launch (0: what would fit in 34 GB of planes)")
@@ -721,6 +842,8 @@ def main():
         reexec_under_torchrun(args, sys.argv[1:])
     if args.workload == "P4":
         run_p4(args)
+    elif args.workload in ("F8", "F9", "F10"):
+        run_efficiency(args)
     else:
         run_ours(args)
 

@@ -74,7 +74,9 @@ class Workload:
     llp_tracks: Tuple[int, int] = (4, 4)
     llp_pt: Tuple[float, float] = (1.0, 10.0)
     llp_half_angle: float = 0.3
+    llp_half_angle_range: Optional[Tuple[float, float]] = None   # if set: drawn per vertex, replaces llp_half_angle
     hit_sigma_mm: float = 0.02                      # azimuthal smearing of a hit: N(0,1) * hit_sigma_mm / r  (R27)
+    vote_flags: int = 0                             # hough_config.vote_flags the workload is meant to be run with
 
     @property
     def n_layers(self) -> int:
@@ -120,6 +122,35 @@ def paper_timing(n_tracks: int, n_events: int = 32) -> Workload:
     expects "7 or more hits per track".  pT is not stated: 1 + Exp(2) GeV as in the other configs."""
     return Workload(f"P4-{n_tracks}", 40, n_events, TRACKER_PAPER, 1, 2048, 2048, l_min=7, max_peaks=16384,
                     n_prompt=(n_tracks, n_tracks), prompt_pt="exp2_trunc1", n_noise=(0, 0), hit_sigma_mm=0.4)
+
+
+def paper_efficiency(kind: str, x: int, n_events: int = 64) -> Workload:
+    """The paper's three efficiency studies (section 7) on its toy detector (ten layers, 0.4 mm):
+      "F8"  one displaced jet of x tracks, nothing else (Fig. 8: efficiency vs tracks per jet);
+      "F9"  x displaced jets of 10 tracks each, nothing else (Fig. 9: efficiency vs jets per event);
+      "F10" 3,000 tracks in total, x displaced jets of 10 tracks among them, the rest prompt (Fig. 10).
+    Every track has 10 hits, so a displaced vertex lies between the 30 mm beam pipe and the first
+    layer (137 mm): R_v uniform in [40, 130] mm.  "Dispersion angles between 15 and 60 degrees" is read
+    as the full opening angle of a jet: its tracks leave the vertex within +- half of it around the radial direction.
+    Not stated in the paper and chosen here (R43): jet-track pT uniform 1-30 GeV, prompt pT 1 + Exp(2) GeV, a
+    3D accumulator of 64 d0 bins over [-80, 80] mm x 1024 x 512 voted with the forward-hemisphere cut and kappa-range
+    filling (vote_flags 3), tracks = peaks with all 10 layers (with filled bands a lower threshold multiplies the
+    duplicate peaks per track), vertices of 7 or more tracks (the paper's "7 or more", "simple reuse" of
+    the peak finder's threshold) on a 256 x 128 (phi_v, R_v) grid over [30, 430) mm."""
+    deg = np.pi / 180.0
+    base = dict(n_events=n_events, radii=TRACKER_PAPER, n_d0=64, n_phi0=1024, n_kappa=512, d0_min=-80.0, d0_max=80.0,
+                l_min=10, max_peaks=16384, max_jets=256, d0_cut_mm=2.5, vtx_n_min=7, max_vertices=64, n_noise=(0, 0),
+                vote_flags=3,
+                prompt_pt="exp2_trunc1", llp_radius=(40.0, 130.0), llp_pt=(1.0, 30.0), hit_sigma_mm=0.4,
+                llp_half_angle_range=(7.5 * deg, 30.0 * deg))
+    if kind == "F8":
+        return Workload(f"F8-{x}", 80, n_prompt=(0, 0), n_llp=(1, 1), llp_tracks=(x, x), **base)
+    if kind == "F9":
+        return Workload(f"F9-{x}", 90, n_prompt=(0, 0), n_llp=(x, x), llp_tracks=(10, 10), **base)
+    if kind == "F10":
+        base["max_peaks"] = 65536
+        return Workload(f"F10-{x}", 100, n_prompt=(3000 - 10 * x, 3000 - 10 * x), n_llp=(x, x), llp_tracks=(10, 10), **base)
+    raise ValueError("kind must be F8, F9 or F10")
 
 
 def scaled(w: Workload, **kw) -> Workload:
@@ -250,7 +281,8 @@ def generate_event(w: Workload, k: int, seed: Optional[int] = None):
     d_v, d_psi, d_kap, d_rv = [], [], [], []
     for j in range(n_v):
         n_t = _randint_incl(rng, w.llp_tracks)
-        d_psi.append(v_phi[j] + rng.uniform(-w.llp_half_angle, w.llp_half_angle, n_t))
+        half = w.llp_half_angle if w.llp_half_angle_range is None else rng.uniform(*w.llp_half_angle_range)
+        d_psi.append(v_phi[j] + rng.uniform(-half, half, n_t))
         dq = rng.choice(np.array([-1.0, 1.0]), n_t)
         dpt = rng.uniform(w.llp_pt[0], w.llp_pt[1], n_t)
         d_kap.append(-dq * 0.3e-3 * w.b_tesla / dpt)

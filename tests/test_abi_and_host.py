@@ -219,6 +219,29 @@ def test_bench_gpus_flag_is_checked_against_the_launch():
     assert bench.gather_event_results.__doc__ and bench.reexec_under_torchrun.__doc__
 
 
+def test_efficiency_workloads_and_truth_matching():
+    """paper_efficiency: ten hits per track on the ten-layer toy detector, x tracks per jet / x jets /
+    3000 tracks in total; bench.match_vertices counts a simulated jet as found iff a vertex lies within the tolerance."""
+    import bench
+    from paper_1309_6275_b200 import workloads as W
+    w = W.paper_efficiency("F8", 6, 4)
+    b = W.generate(w, keep_truth=True)
+    assert b.n_hits == 4 * 6 * 10 and all(t["n_vertices"] == 1 for t in b.truth)
+    assert all(40.0 <= t["vertex_r"][0] <= 130.0 for t in b.truth) and w.n_layers == 10 and w.vote_flags == 3
+    w = W.paper_efficiency("F9", 5, 2)
+    assert W.generate(w).n_hits == 2 * 5 * 10 * 10
+    w = W.paper_efficiency("F10", 7, 1)
+    b = W.generate(w, keep_truth=True)
+    assert abs(b.n_hits - 30000) <= 300 and b.truth[0]["prompt_pt"].size == 3000 - 70     # a few 1 GeV loopers miss a layer
+    # matching: vertices at (100 mm, 0) and (50 mm, pi/2); found ones 3 mm, 30 mm and far away
+    tr, tp = np.array([100.0, 50.0]), np.array([0.0, np.pi / 2])
+    fr, fp = np.array([103.0, 80.0, 200.0]), np.array([0.0, np.pi / 2, 3.0])
+    assert bench.match_vertices(fr, fp, tr, tp, 10.0) == (1, 2)
+    assert bench.match_vertices(fr, fp, tr, tp, 31.0) == (2, 1)
+    assert bench.match_vertices(np.zeros(0), np.zeros(0), tr, tp, 10.0) == (0, 0)
+    assert bench.match_vertices(fr, fp, np.zeros(0), np.zeros(0), 10.0) == (0, 3)
+
+
 def test_o2_instruction_count():
     """bench.py's FP32 roofline term uses I_FP32 = FMA-pipe instructions (FADD / FMUL / FFMA) of the plain O-2 function
     compiled for sm_100a.  Recount them from the SASS of csrc/o2_count.cu: fast path only (up to the
