@@ -139,7 +139,7 @@ def paper_efficiency(kind: str, x: int, n_events: int = 64) -> Workload:
     the peak finder's threshold) on a 256 x 128 (phi_v, R_v) grid over [30, 430) mm."""
     deg = np.pi / 180.0
     base = dict(n_events=n_events, radii=TRACKER_PAPER, n_d0=64, n_phi0=1024, n_kappa=512, d0_min=-80.0, d0_max=80.0,
-                l_min=10, max_peaks=16384, max_jets=256, d0_cut_mm=2.5, vtx_n_min=7, max_vertices=64, n_noise=(0, 0),
+                l_min=10, max_peaks=16384, max_jets=256, d0_cut_mm=2.5, vtx_n_min=7, max_vertices=256, n_noise=(0, 0),
                 vote_flags=3,
                 prompt_pt="exp2_trunc1", llp_radius=(40.0, 130.0), llp_pt=(1.0, 30.0), hit_sigma_mm=0.4,
                 llp_half_angle_range=(7.5 * deg, 30.0 * deg))
