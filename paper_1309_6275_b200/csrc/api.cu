@@ -252,6 +252,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     }
     A(cudaMemset(c->d_status, 0, 8));
     A(cudaMemset(c->d_tilectr, 0, 8));
+    // all-empty windows until the first call with hits computes them (build_windows_kernel skips unchanged r ranges)
+    A(cudaMemset(c->d_tilewin, 0, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips * sizeof(TileWin)));
     A(cudaMemset(c->d_cand_n, 0, (size_t)c->fused_events * 4));
     if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
     *out = c;

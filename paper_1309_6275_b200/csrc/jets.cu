@@ -1,4 +1,5 @@
-// A5 peak -> track conversion and A6 seeded phi-cone track-jets, one warp per event (sm_100a).
+// A5 peak -> track conversion and A6 seeded phi-cone track-jets, one warp per event (sm_100a); for small batches
+// (single-event latency) one block of 8 warps per event.
 //
 // DESIGN.md O-4 / O-5 (PAPER.md:87 transverse-momentum measurement; PAPER.md:113-123 jets and the
 // interaction-point remark; clustering rule from north_star as read in R17-R22).  All decisions are taken on
@@ -32,14 +33,20 @@ __device__ __forceinline__ uint64_t warp_min_u64(uint64_t v)
     return v;
 }
 
-// one warp (= one block) per event; the clustering keys live in shared memory when the event's tracks fit
-// (kSmemKeys of them), else in the context's global workspace
+// one block of NW warps per event (NW = 1: large batches, many events per SM; NW = 8: a handful of events, where the
+// length of the per-jet passes over the tracks is what counts); the clustering keys live in shared memory when the
+// event's tracks fit (kSmemKeys of them), else in the context's global workspace
 constexpr uint32_t kSmemKeys = 4096;
 
-__global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
+template <int NW>
+__global__ void __launch_bounds__(32 * NW) jets_kernel(const JetParams p)
 {
     __shared__ uint64_t s_keys[kSmemKeys];
-    const int lane = threadIdx.x & 31;
+    __shared__ uint64_t s_best[NW];
+    __shared__ uint32_t s_cnt[NW][2];
+    __shared__ double s_pt[NW];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr uint32_t NT = 32u * NW;
     const uint32_t e = blockIdx.x;
     if (e >= p.n_events) return;
     const uint32_t np_e = p.n_peaks[e];
@@ -50,10 +57,11 @@ __global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
     uint64_t* keys = (T <= kSmemKeys) ? s_keys : p.keys + (size_t)e * p.max_peaks;
     const int NK = p.n_kappa, N = p.n_phi0;
     const double kmax = (double)p.kmax;
+    auto block_sync = [&]() { if (NW == 1) __syncwarp(); else __syncthreads(); };
 
     // A5: tracks, and the integer keys of the clustering: [63] assigned, [32..55] a = |2 ik - (NK-1)|,
     // [1..21] ip, [0] displaced
-    for (uint32_t j = lane; j < T; j += 32) {
+    for (uint32_t j = tid; j < T; j += NT) {
         const uint32_t lin = pk[j].lin;
         const uint32_t ik = lin % (uint32_t)NK, t = lin / (uint32_t)NK;
         const uint32_t ip = t % (uint32_t)N, id = t / (uint32_t)N;
@@ -70,14 +78,14 @@ __global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
         const uint32_t disp = (p.n_d0 > 1 && fabsf(d0) > p.d0_cut) ? 1u : 0u;
         keys[j] = ((uint64_t)a << 32) | ((uint64_t)ip << 1) | disp;
     }
-    __syncwarp();
+    block_sync();
 
     // A6: repeat { seed = unassigned track with the smallest (a, j); members = unassigned within the cone }
     uint32_t J = 0;
     bool any_flag = false;
     for (;;) {
         uint64_t best = ~0ull;
-        for (uint32_t j = lane; j < T; j += 32) {
+        for (uint32_t j = tid; j < T; j += NT) {
             const uint64_t k = keys[j];
             if (!(k & KEY_ASSIGNED)) {
                 const uint64_t cand = (k & 0x00ffffff00000000ull) | j;
@@ -85,12 +93,19 @@ __global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
             }
         }
         best = warp_min_u64(best);
-        if (best == ~0ull) break;
+        if (NW > 1) {
+            if (lane == 0) s_best[warp] = best;
+            __syncthreads();
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { const uint64_t o = s_best[w]; best = (o < best) ? o : best; }
+        }
+        if (best == ~0ull) break;                                // block-uniform
         const uint32_t seed = (uint32_t)(best & 0xffffffffu);
         const int ip_seed = (int)((keys[seed] >> 1) & 0xfffffu);
+        block_sync();                                            // every thread has read the seed's key
         uint32_t n_tracks = 0, n_disp = 0;
         double sum_pt = 0.0;
-        for (uint32_t j = lane; j < T; j += 32) {
+        for (uint32_t j = tid; j < T; j += NT) {
             const uint64_t k = keys[j];
             if (k & KEY_ASSIGNED) continue;
             int d = abs((int)((k >> 1) & 0xfffffu) - ip_seed);
@@ -103,14 +118,22 @@ __global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
                 if (J < p.max_jets) trk[j].jet = (int32_t)J;
             }
         }
-        __syncwarp();
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
             n_tracks += __shfl_xor_sync(0xffffffffu, n_tracks, d);
             n_disp += __shfl_xor_sync(0xffffffffu, n_disp, d);
             sum_pt += __shfl_xor_sync(0xffffffffu, sum_pt, d);
         }
-        if (lane == 0 && J < p.max_jets) {
+        if (NW > 1) {
+            if (lane == 0) { s_cnt[warp][0] = n_tracks; s_cnt[warp][1] = n_disp; s_pt[warp] = sum_pt; }
+            __syncthreads();                                     // also orders the key updates before the next round
+            n_tracks = 0; n_disp = 0; sum_pt = 0.0;
+#pragma unroll
+            for (int w = 0; w < NW; ++w) { n_tracks += s_cnt[w][0]; n_disp += s_cnt[w][1]; sum_pt += s_pt[w]; }
+        } else {
+            __syncwarp();
+        }
+        if (tid == 0 && J < p.max_jets) {
             hough_jet jt;
             jt.seed_track = seed; jt.n_tracks = n_tracks; jt.n_displaced = n_disp;
             jt.phi = trk[seed].phi0; jt.sum_pt = (float)sum_pt;
@@ -119,7 +142,7 @@ __global__ void __launch_bounds__(32) jets_kernel(const JetParams p)
         any_flag = any_flag || (n_disp >= p.n_min);
         ++J;
     }
-    if (lane == 0) { p.n_jets[e] = J; p.flag[e] = any_flag ? 1 : 0; }
+    if (tid == 0) { p.n_jets[e] = J; p.flag[e] = any_flag ? 1 : 0; }
 }
 
 }  // namespace
@@ -135,7 +158,9 @@ cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_pea
     p.n_events = n_events; p.max_peaks = c->cfg.max_peaks_per_event; p.max_jets = c->cfg.max_jets_per_event;
     p.n_d0 = (int)c->cfg.n_d0; p.n_phi0 = (int)c->cfg.n_phi0; p.n_kappa = (int)c->cfg.n_kappa;
     p.kmax = c->kmax; p.b_tesla = c->cfg.b_tesla; p.d0_cut = d0_cut; p.cone_bins = cone_bins; p.n_min = n_min;
-    jets_kernel<<<n_events, 32, 0, st>>>(p);
+    // few events (single-event latency): eight warps share an event's passes over its tracks
+    if (n_events < 64) jets_kernel<8><<<n_events, 256, 0, st>>>(p);
+    else jets_kernel<1><<<n_events, 32, 0, st>>>(p);
     ++c->launches;
     return cudaGetLastError();
 }

@@ -21,7 +21,7 @@
 
 namespace {
 
-constexpr int kVtxThreads = 512;
+constexpr int kVtxThreads = 1024;
 
 struct VtxParams {
     const hough_peak* peaks; const uint32_t* n_peaks;
