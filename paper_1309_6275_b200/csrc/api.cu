@@ -38,7 +38,7 @@ void free_all(hough_ctx* c)
 {
     cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
     cudaFree(c->d_rec); cudaFree(c->d_rec_u); cudaFree(c->d_key); cudaFree(c->d_seg); cudaFree(c->d_btab);
-    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_status); cudaFree(c->d_tilectr);
+    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_tilewin_mo); cudaFree(c->d_redo); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_cand); cudaFree(c->d_cand_n); cudaFree(c->d_sortkeys);
     cudaFree(c->d_ce); cudaFree(c->d_se);
@@ -170,6 +170,11 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         mirror_ok = c0[ip + NP / 2] == -c0[ip] && s0[ip + NP / 2] == -s0[ip];
     for (uint32_t id = 0; mirror_ok && id < ND; ++id) mirror_ok = d0c[ND - 1 - id] == -d0c[id];
     if (plan_vote(c, mirror_ok) != cudaSuccess || plan_peaks(c) != cudaSuccess) { delete c; return HOUGH_EUNSUPPORTED; }
+    // fused path: which tiles hough_vote_peaks uses on a grid that has both kinds (debug / test switch, read once):
+    // HOUGH_FUSED_TILES=count -> count + mask tiles, =mask -> mask-only tiles, unset -> chosen per call by occupancy
+    c->fused_scheme = 0;
+    if (const char* ft = getenv("HOUGH_FUSED_TILES")) c->fused_scheme = (ft[0] == 'c') ? 1 : (ft[0] == 'm') ? 2 : 0;
+    c->prep_hits_per_event = 0.0;
     // the branch-free exact division of the vote kernel is only used inside this range (vote.cu, div_rn_tame)
     c->tame_tables = cfg->kappa_max >= 9.094947e-13f && cfg->kappa_max <= 1.0995116e12f;      // [2^-40, 2^40]
     for (uint32_t id = 0; id < ND; ++id) {
@@ -193,6 +198,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
     A(dev_alloc(&c->d_layer_r, 4 * HOUGH_MAX_LAYERS));   // live min / max per layer + the copy the recount reads
     A(dev_alloc(&c->d_tilewin, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips));
+    if (c->has_mo) A(dev_alloc(&c->d_tilewin_mo, (size_t)c->vote_mo.nk_seg * HOUGH_MAX_LAYERS * c->vote_mo.n_strips));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_tilectr, 2));
     A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
@@ -209,6 +215,7 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     }
     A(dev_alloc(&c->d_cand, (size_t)c->fused_events * c->cand_cap));
     A(dev_alloc(&c->d_cand_n, c->fused_events));
+    A(dev_alloc(&c->d_redo, (size_t)c->fused_events + 1));
     A(dev_alloc(&c->d_sortkeys, (size_t)c->fused_events * c->cand_cap_pow2));
     if (cfg->host_chunk_events > 0) {
         const size_t E = cfg->max_events, H = cfg->max_hits;
@@ -254,6 +261,8 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(cudaMemset(c->d_tilectr, 0, 8));
     // all-empty windows until the first call with hits computes them (build_windows_kernel skips unchanged r ranges)
     A(cudaMemset(c->d_tilewin, 0, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips * sizeof(TileWin)));
+    if (c->has_mo)
+        A(cudaMemset(c->d_tilewin_mo, 0, (size_t)c->vote_mo.nk_seg * HOUGH_MAX_LAYERS * c->vote_mo.n_strips * sizeof(TileWin)));
     A(cudaMemset(c->d_cand_n, 0, (size_t)c->fused_events * 4));
     if (err != cudaSuccess) { cuda_fail(err, "hough_create upload"); free_all(c); delete c; return HOUGH_ECUDA; }
     *out = c;

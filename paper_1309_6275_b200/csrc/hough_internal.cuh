@@ -67,6 +67,7 @@ struct hough_ctx {
     uint16_t* d_btab;                         // [max_events][16][nb + 1] bucket starts relative to the layer segment
     uint32_t* d_layer_r;                      // [4*16] float bits: min r, max r per layer (live), then the last call's copy
     TileWin* d_tilewin;                       // [nk_seg][16][n_strips]
+    TileWin* d_tilewin_mo;                    // the same for the mask-tile plan of the fused path (vote_mo), if any
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
     uint32_t* d_tilectr;                      // [2]: vote kernel tile ticket + finished-block count (zero between launches)
     uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
@@ -90,6 +91,11 @@ struct hough_ctx {
     std::vector<int> ev_label;                // stage that STARTS at the mark (0 prep, 1 vote, 2 peaks, 3 jets, 4 vertices), -1: end of a call
     size_t ev_used;
     VotePlan vote;
+    VotePlan vote_mo;                         // fused path, mask-only mirror tiles (has_mo): larger kappa range per tile
+    bool has_mo;
+    int fused_scheme;                         // 0: choose per call by occupancy, 1: count + mask tiles, 2: mask tiles (HOUGH_FUSED_TILES)
+    double prep_hits_per_event;               // mean hits per event of the last launch_prep (tile choice of the fused path)
+    uint32_t* d_redo;                         // [1 + fused_events]: number and indices of the events whose mask-tile candidates overflowed
     PeakPlan peak;
     cudaStream_t last_stream;
     uint64_t launches;

@@ -81,13 +81,13 @@ def test_packed_sweep_keeps_every_rounding_of_o2():
     from paper_1309_6275_b200 import build
     lib = build.build()
     sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
-    # vote_kernel<MODE3D, KL, FUSED, MIRROR, VARIANT>: the packed 3D kernels (the scalar voting-variant kernels are left out)
+    # vote_kernel<MODE3D, KL, FUSED, MIRROR, VARIANT, MO>: the packed 3D kernels (the scalar voting-variant kernels are left out)
     kernels = []
     for body in sass.split("Function : ")[1:]:
-        m = re.search(r"vote_kernelILb(\d)ELi(\d)ELb(\d)ELb(\d)ELb(\d)EEEv", body.split("\n")[0])
+        m = re.search(r"vote_kernelILb(\d)ELi(\d)ELb(\d)ELb(\d)ELb(\d)ELb(\d)EEEv", body.split("\n")[0])
         if m and m.group(1) == "1" and m.group(5) == "0":
             kernels.append((m.group(4) == "1", body))
-    assert len(kernels) == 8                                     # KL = 1, 2, 4 x {planes, fused} + the two mirror kernels
+    assert len(kernels) == 9                     # KL = 1, 2, 4 x {planes, fused} + the mirror kernels (planes, fused, fused mask tiles)
     n_mirror = 0
     for mirror, body in kernels:
         n_rm = len(re.findall(r"\bFADD2\.RM\b", body))
@@ -102,7 +102,7 @@ def test_packed_sweep_keeps_every_rounding_of_o2():
             assert n_add == 3 * n_rm, (n_add, n_rm)
             assert n_mul == 2 * n_rm, (n_mul, n_rm)
             assert n_fma == 5 * n_rm, (n_fma, n_rm)
-    assert n_mirror == 2
+    assert n_mirror == 3
 
 
 def test_product_path_never_touches_the_oracle():
