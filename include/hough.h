@@ -143,13 +143,19 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
  * identified by finding local maxima", and PAPER.md:109: the transform is limited "more by memory access
  * operations rather than the computational rate").  Same result as hough_vote followed by hough_peaks -- the same
  * peaks, in ascending lin, with the same count / mask, and the true total -- but the vote kernel finds the peak
- * candidates (popcount(mask) >= l_min) while its tile is in shared memory, compares them with the neighbours
- * inside the tile, and a second kernel recomputes, from the hits, the few neighbour bins that lie across a tile
- * border (O-2 verbatim, so the counts are the accumulator's).  No plane is written.
+ * candidates (popcount(mask) >= l_min) while its tile is in shared memory and a second kernel recomputes, from the
+ * hits, the counts it needs (O-2 verbatim, so the counts are the accumulator's).  No plane is written.  Two kinds
+ * of tile: "mask tiles" accumulate only the layer masks (one shared reduction per vote, twice the
+ * kappa range per tile) and have the count of every candidate and of its 26 neighbours recomputed; "count + mask
+ * tiles" accumulate both, compare a candidate with its neighbours inside the tile and have only the neighbours
+ * across a tile border recomputed.  A call starts with mask tiles when the grid allows them (mirror-symmetric
+ * tables) and few chance candidates are expected, and votes the events whose candidates overflow the buffer again
+ * with count + mask tiles, on the device; the result does not depend on the kind of tile (environment variable
+ * HOUGH_FUSED_TILES=mask|count, read by hough_create, forces one: tests).
  *   arguments as hough_vote / hough_peaks.  Capacity: if an event has more than max_candidates_per_event
- *   candidates, HOUGH_ST_CANDIDATE_OVERFLOW is raised and d_n_peaks[e] = HOUGH_N_PEAKS_OVERFLOW (no record of
- *   that event is valid; hough_jets treats it as an event without tracks): re-run such events through
- *   hough_vote + hough_peaks (hough_trigger_host does).
+ *   candidates (count + mask tiles), HOUGH_ST_CANDIDATE_OVERFLOW is raised and d_n_peaks[e] =
+ *   HOUGH_N_PEAKS_OVERFLOW (no record of that event is valid; hough_jets treats it as an event without tracks):
+ *   re-run such events through hough_vote + hough_peaks (hough_trigger_host does).
  * Returns HOUGH_EINVAL as hough_vote / hough_peaks do, and if n_events exceeds the fused capacity
  * (host_chunk_events if that is > 0, else max_events).
  */
