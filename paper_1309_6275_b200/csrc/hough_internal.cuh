@@ -22,7 +22,8 @@ struct TileWin { int a0, len0, a1, len1; };
 constexpr int kSegStride = HOUGH_MAX_LAYERS + 2;
 
 // Fused path: one peak candidate found in a vote tile.  cm = count | mask << 16; need = neighbour columns the tile
-// could not check, bit (dd+1)*3 + (dp+1); state = 0 pending the recount, 1 confirmed peak, 2 rejected.
+// could not check, bit (dd+1)*3 + (dp+1), and bit 9 = "count not known yet" (mask tiles: the recount fills it in);
+// state = 0 pending the recount, 1 confirmed peak, 2 rejected.
 struct PeakCand { uint32_t lin, cm, need, state; };
 
 struct VotePlan {
