@@ -901,3 +901,26 @@ def test_p20_filled_bands_match_an_fp64_evaluation_at_the_column_edges():
     assert ok.sum() > 0.9 * ok.size
     assert np.array_equal(cf.astype(np.int64)[ok], ref[ok])
     assert vf > 2 * O.vote_variant(g, O.VOTE_HEMI, r, phi, lay)[2]
+
+
+# ----------------------------------------------------------------------------------------------
+# regression fixture of the oracle (tests/golden/; written by a committed script that calls only oracle/)
+# ----------------------------------------------------------------------------------------------
+
+def test_oracle_matches_its_golden_fixture():
+    """tests/golden/oracle_regression.json (see tests/golden/README.md): not paper values -- the paper prints none -- but
+    the oracle's own outputs on four small seeded events, so that an unintended change of its arithmetic, of a reading or
+    of the generator is noticed."""
+    import importlib.util
+    import json
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_fixtures", os.path.join(here, "make_oracle_fixtures.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    stored = json.load(open(os.path.join(here, "oracle_regression.json")))
+    now = mod.make()
+    assert len(stored) == len(now) == 4
+    for a, b in zip(stored, now):
+        assert a == b, (a["case"], {k: (a[k], b[k]) for k in a if a[k] != b[k]})
+
