@@ -38,7 +38,7 @@ void free_all(hough_ctx* c)
 {
     cudaFree(c->d_c0); cudaFree(c->d_s0); cudaFree(c->d_d0c); cudaFree(c->d_two_d0); cudaFree(c->d_d0sq);
     cudaFree(c->d_rec); cudaFree(c->d_rec_u); cudaFree(c->d_key); cudaFree(c->d_seg); cudaFree(c->d_btab);
-    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_tilewin_mo); cudaFree(c->d_redo); cudaFree(c->d_status); cudaFree(c->d_tilectr);
+    cudaFree(c->d_layer_r); cudaFree(c->d_tilewin); cudaFree(c->d_tilewin_mo); cudaFree(c->d_redo); cudaFree(c->d_vtx_gplane); cudaFree(c->d_vtx_done); cudaFree(c->d_status); cudaFree(c->d_tilectr);
     cudaFree(c->d_bitmap); cudaFree(c->d_grpcnt); cudaFree(c->d_jetkeys);
     cudaFree(c->d_cand); cudaFree(c->d_cand_n); cudaFree(c->d_sortkeys);
     cudaFree(c->d_ce); cudaFree(c->d_se);
@@ -193,6 +193,10 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     A(dev_alloc(&c->d_kc, NK));
     A(dev_alloc(&c->d_ce, NP)); A(dev_alloc(&c->d_se, NP));
     A(dev_alloc(&c->d_vex, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vey, cfg->n_vtx_phi)); A(dev_alloc(&c->d_vrc, cfg->n_vtx_r));
+    if (cfg->n_vtx_phi) {
+        A(dev_alloc(&c->d_vtx_gplane, (size_t)kVtxSplitEvents * cfg->n_vtx_phi * cfg->n_vtx_r / 2));
+        A(dev_alloc(&c->d_vtx_done, kVtxSplitEvents));
+    }
     A(dev_alloc(&c->d_rec, cfg->max_hits)); A(dev_alloc(&c->d_rec_u, cfg->max_hits)); A(dev_alloc(&c->d_key, cfg->max_hits));
     A(dev_alloc(&c->d_seg, (size_t)cfg->max_events * kSegStride));
     A(dev_alloc(&c->d_btab, (size_t)cfg->max_events * HOUGH_MAX_LAYERS * (c->vote.nb + 1)));
@@ -259,6 +263,10 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     }
     A(cudaMemset(c->d_status, 0, 8));
     A(cudaMemset(c->d_tilectr, 0, 8));
+    if (cfg->n_vtx_phi) {
+        A(cudaMemset(c->d_vtx_gplane, 0, (size_t)kVtxSplitEvents * cfg->n_vtx_phi * cfg->n_vtx_r * 2));
+        A(cudaMemset(c->d_vtx_done, 0, kVtxSplitEvents * 4));
+    }
     // all-empty windows until the first call with hits computes them (build_windows_kernel skips unchanged r ranges)
     A(cudaMemset(c->d_tilewin, 0, (size_t)c->vote.nk_seg * HOUGH_MAX_LAYERS * c->vote.n_strips * sizeof(TileWin)));
     if (c->has_mo)

@@ -11,6 +11,10 @@
 
 #define HOUGH_MAX_LAYERS 16
 
+// hough_vertices on at most kVtxSplitEvents events runs kVtxSplit blocks per event (single-event latency)
+constexpr uint32_t kVtxSplitEvents = 8;
+constexpr uint32_t kVtxSplit = 16;
+
 // Prepared hit record (float4): {RN32(sin phi), RN32(cos phi), r, bits}, bits = (0x10000 << layer) | wild, where
 // "wild" marks a hit whose r is outside [2^-20, 2^20] or not finite (no window pruning, generic IEEE division).
 
@@ -59,6 +63,8 @@ struct hough_ctx {
     float* d_kc;                              // [NK] kappa bin centres, fp32 rounded once from double (O-6)
     float* d_vex; float* d_vey;               // [n_vtx_phi] phi_v bin-edge directions (cos, sin)(k * 2pi / n_vtx_phi)
     float* d_vrc;                             // [n_vtx_r] R_v bin centres
+    uint32_t* d_vtx_gplane;                   // [kVtxSplitEvents][n_vtx_phi * n_vtx_r / 2] vertex planes of the split kernel (zero between calls)
+    uint32_t* d_vtx_done;                     // [kVtxSplitEvents] finished-block counters of the split kernel (zero between calls)
     bool tame_tables;                         // d0 centres and kappa_max inside the range div_rn_tame is proven for
     // per-call workspace
     float4* d_rec_u;                          // [max_hits] prepared hits in input order (sort scratch)

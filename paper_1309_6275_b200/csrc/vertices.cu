@@ -34,6 +34,11 @@ struct VtxParams {
     float d0_cut;
     uint32_t n_min;
     double dphi_v;
+    // SPLIT kernel (a handful of events: single-event latency): `split` blocks share an event's tracks and vote into the
+    // event's plane in global memory; the last block to finish takes the plane into shared memory and finds the peaks
+    uint32_t split;
+    uint32_t* gplane;                // [kVtxSplitEvents][bins / 2], zero between calls
+    uint32_t* done;                  // [kVtxSplitEvents], zero between calls
 };
 
 __device__ __forceinline__ uint32_t angle_bin(const float* ex, const float* ey, int n_vphi, float x, float y)
@@ -78,13 +83,17 @@ __device__ __forceinline__ bool vtx_is_peak(const uint32_t* acc, int NPV, int NR
     return true;
 }
 
+template <bool SPLIT>
 __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
 {
     extern __shared__ uint32_t acc[];                            // [n_vphi * n_vr / 2]: two 16-bit counts per word, then tables
     __shared__ uint32_t s_warp[kVtxThreads / 32];
     __shared__ uint32_t s_total;
+    __shared__ uint32_t s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t e = blockIdx.x;
+    const uint32_t e = SPLIT ? blockIdx.x / p.split : blockIdx.x;
+    const uint32_t sub = SPLIT ? blockIdx.x - e * p.split : 0u;
+    const uint32_t n_sub = SPLIT ? p.split : 1u;
     const int NPV = p.n_vphi, NR = p.n_vr;
     const uint32_t bins = (uint32_t)NPV * (uint32_t)NR;
     // the edge directions (binary-searched per vote) and the R_v centres live in shared memory behind the accumulator
@@ -100,7 +109,8 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
     const uint32_t T = (np_e == HOUGH_N_PEAKS_OVERFLOW) ? 0u : min(np_e, p.max_peaks);
     const hough_peak* pk = p.peaks + (size_t)e * p.max_peaks;
     // ---- O-6: one warp per track, lanes over the R_v bins ----
-    for (uint32_t j = warp; j < T; j += kVtxThreads / 32) {
+    uint32_t* const vote_plane = SPLIT ? p.gplane + (size_t)e * (bins / 2) : acc;
+    for (uint32_t j = sub * (kVtxThreads / 32) + warp; j < T; j += n_sub * (kVtxThreads / 32)) {
         const uint32_t lin = pk[j].lin;
         const uint32_t ik = lin % (uint32_t)p.n_kappa, t = lin / (uint32_t)p.n_kappa;
         const uint32_t ip = t % (uint32_t)p.n_phi0, id = t / (uint32_t)p.n_phi0;
@@ -122,8 +132,19 @@ __global__ void __launch_bounds__(kVtxThreads) vertex_kernel(const VtxParams p)
             const float x = __fsub_rn(__fmul_rn(c0, cd), __fmul_rn(s0, s));
             const float y = __fadd_rn(__fmul_rn(s0, cd), __fmul_rn(c0, s));
             const uint32_t b = angle_bin(s_ex, s_ey, NPV, x, y) * (uint32_t)NR + (uint32_t)ir;
-            atomicAdd(&acc[b >> 1], 1u << (16u * (b & 1u)));
+            atomicAdd(&vote_plane[b >> 1], 1u << (16u * (b & 1u)));
         }
+    }
+    if (SPLIT) {
+        // the last block of the event to get here takes the finished plane into shared memory (and leaves zeros behind)
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) s_last = (atomicAdd(p.done + e, 1u) == p.split - 1u) ? 1u : 0u;
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+        for (uint32_t i = tid; i < bins / 2; i += kVtxThreads) { acc[i] = __ldcg(vote_plane + i); vote_plane[i] = 0u; }
+        if (tid == 0) p.done[e] = 0u;
     }
     __syncthreads();
     if (p.plane) {                                               // optional: the vertex plane itself (tests)
@@ -205,9 +226,15 @@ cudaError_t launch_vertices(hough_ctx* c, uint32_t n_events, const hough_peak* d
     p.dphi_v = 6.283185307179586476925286766559 / (double)c->cfg.n_vtx_phi;
     const size_t bins = (size_t)c->cfg.n_vtx_phi * c->cfg.n_vtx_r;
     const size_t smem = bins * 2 + (2 * (size_t)c->cfg.n_vtx_phi + c->cfg.n_vtx_r) * 4 + bins / 32 * 4;
-    cudaError_t err = cudaFuncSetAttribute(vertex_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // a handful of events (single-event latency): several blocks per event
+    const bool split = n_events <= kVtxSplitEvents && c->d_vtx_gplane != nullptr;
+    p.split = split ? kVtxSplit : 1u;
+    p.gplane = c->d_vtx_gplane; p.done = c->d_vtx_done;
+    cudaError_t err = cudaFuncSetAttribute(split ? vertex_kernel<true> : vertex_kernel<false>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return err;
-    vertex_kernel<<<n_events, kVtxThreads, smem, st>>>(p);
+    if (split) vertex_kernel<true><<<n_events * kVtxSplit, kVtxThreads, smem, st>>>(p);
+    else vertex_kernel<false><<<n_events, kVtxThreads, smem, st>>>(p);
     ++c->launches;
     return cudaGetLastError();
 }
