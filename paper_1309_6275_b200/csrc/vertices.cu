@@ -9,6 +9,8 @@
 //
 // One block per event; the whole vertex accumulator (phi_v x R_v bins, 16-bit counts, two per 32-bit word) lives in
 // shared memory, so nothing but the peak list of the first transform is read and nothing but the vertex list written.
+// (Calls with at most kVtxSplitEvents events -- single-event latency -- run kVtxSplit blocks per event instead, which
+// vote into the event's plane in global memory; the last block to finish takes it into shared memory for O-7.)
 //   O-6  a warp takes a track (bin-centre parameters d0c, (cos, sin) phi0c, kappa_c of its peak), its lanes the R_v
 //        bins: s = (kappa (r^2 + d0^2) - 2 d0) / (2 r (1 - kappa d0)) with IEEE division, the crossing direction by
 //        rotating (cos phi0, sin phi0) by (sqrt(1 - s^2), s) with IEEE sqrt, the phi_v bin by a cross-product binary
