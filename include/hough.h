@@ -13,8 +13,8 @@
  * cudaStream_t passed as void*.  All work is enqueued on `stream`; only hough_create, hough_destroy,
  * hough_status, hough_trigger_host and hough_microbench synchronise.  Calls on one context must be
  * stream-ordered by the caller (the context owns a per-call workspace).  No entry point allocates or
- * frees device memory except hough_create / hough_destroy.  There is no CPU fallback anywhere: without a
- * CUDA device hough_create fails with HOUGH_ECUDA.
+ * frees device memory except hough_create / hough_destroy (hough_jets_static needs neither of them).
+ * There is no CPU fallback anywhere: without a CUDA device hough_create fails with HOUGH_ECUDA.
  *
  * Notation: E events; ND, NPHI, NK bins in d0, phi0, kappa; bin (id, ip, ik) has linear index
  * lin = (id*NPHI + ip)*NK + ik (kappa fastest).  Units: mm, rad, 1/mm, T, GeV.
@@ -77,7 +77,8 @@ enum {
     HOUGH_EINVAL = -1,       /* bad config / null pointer / size over the configured maximum / bad scalar argument */
     HOUGH_ECUDA = -2,        /* CUDA runtime error (text via hough_strerror)                                        */
     HOUGH_ENOMEM = -3,       /* device allocation failed in hough_create                                            */
-    HOUGH_EUNSUPPORTED = -4  /* configuration valid but outside what the kernels are built for                      */
+    HOUGH_EUNSUPPORTED = -4, /* configuration valid but outside what the kernels are built for                      */
+    HOUGH_ETOOLARGE = -5     /* hough_jets_static: the call needs more scratch than the library's fixed array holds  */
 };
 
 /* sticky status bits (hough_status) for conditions only visible on the device; they never trap */
@@ -179,6 +180,40 @@ int hough_vote_peaks(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_of
 int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
                float cone_rad, float d0_cut_mm, uint32_t n_displaced_min,
                hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag, void* stream);
+
+/*
+ * hough_jets without a context and without any allocation -- for callers that are not allowed to allocate.
+ *
+ * Who that is: a trigger process that handed out all of its device memory at start-up and runs under a fixed
+ * budget (a cudaMalloc there fails, or is forbidden by the experiment's framework); a latency-critical loop, where
+ * cudaMalloc / cudaFree would stall every stream of the device; a plug-in hosted by another runtime that owns the
+ * allocator and hands the plug-in nothing but its input and output buffers.  None of them can call hough_create,
+ * which allocates the workspaces of the whole path.  This one call gives them A5-A6 (same definition, same kernel
+ * and same results as hough_jets: PAPER.md:87): it takes the grid description from a HOST
+ * hough_config, the inputs and outputs from the caller, and keeps its two pieces of scratch -- the table of d0 bin
+ * centres and the clustering keys of events with more than 4096 tracks -- in an array that is part of the
+ * library's device image (a file-scope `static __device__` array in csrc/jets.cu, about 4 MB, held by every GPU
+ * that loads the library until the process exits).  It calls no cudaMalloc, cudaFree or allocating library routine.
+ *
+ *   cfg   HOST.  Read: n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, max_peaks_per_event,
+ *         max_jets_per_event (checked as hough_create checks them); every other field is ignored.
+ *   other arguments: DEVICE pointers, exactly as hough_jets.
+ * Limits (the scratch is fixed): n_events * max_peaks_per_event <= HOUGH_JETS_STATIC_MAX_TRACKS and
+ * n_d0 <= HOUGH_JETS_STATIC_MAX_D0; beyond them the call does nothing and returns HOUGH_ETOOLARGE.
+ * HOUGH_EINVAL for a null pointer or a bad cfg / cone_rad / d0_cut_mm; HOUGH_ECUDA as elsewhere.
+ *
+ * Set-up: the first call on each device (with that device current) looks up the device address of the scratch
+ * array once and checks that the device is sm_100-class; make that first call before any stream capture.
+ * Sharing: every call on a device uses the same array.  Nothing in it has to start at zero -- each call writes the
+ * d0 table and every key it later reads -- but it keeps the last call's contents, so two calls that overlap on the
+ * GPU (different streams, no dependency between them) race: order them on one stream or with events.
+ * Asynchronous on `stream` like hough_jets.
+ */
+#define HOUGH_JETS_STATIC_MAX_TRACKS (1u << 19)   /* 524 288 clustering keys of 8 B = 4 MiB */
+#define HOUGH_JETS_STATIC_MAX_D0 4096u            /* d0 bin centres, 16 KiB                 */
+int hough_jets_static(const hough_config* cfg, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                      float cone_rad, float d0_cut_mm, uint32_t n_displaced_min,
+                      hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag, void* stream);
 
 /*
  * The paper's SECOND Hough transform: tracks -> displaced vertices (section 6: "the corresponding

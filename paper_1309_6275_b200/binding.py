@@ -21,12 +21,13 @@ JET_DTYPE = np.dtype([("seed_track", "<u4"), ("n_tracks", "<u4"), ("n_displaced"
                       ("phi", "<f4"), ("sum_pt", "<f4")])
 VERTEX_DTYPE = np.dtype([("r", "<f4"), ("phi", "<f4"), ("n_tracks", "<u4"), ("lin", "<u4")])
 
+JETS_STATIC_MAX_TRACKS, JETS_STATIC_MAX_D0, ETOOLARGE = 1 << 19, 4096, -5
 ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING, ST_CANDIDATE_OVERFLOW = 1, 2, 4, 8
 ST_ERRORS = ST_EVENT_TOO_LARGE | ST_BAD_OFFSETS            # the bits that mean "results undefined"
 N_PEAKS_OVERFLOW = 0xFFFFFFFF
 VOTE_HEMI, VOTE_FILL = 1, 2
 EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_vote_peaks",
-           "hough_jets", "hough_vertices", "hough_trigger_host_vtx",
+           "hough_jets", "hough_jets_static", "hough_vertices", "hough_trigger_host_vtx",
            "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
            "hough_debug_prepared_hits", "hough_debug_div_check", "hough_profile", "hough_profile_read"]
 
@@ -68,6 +69,7 @@ def load_library() -> C.CDLL:
         lib.hough_peaks.argtypes = [p, u32, p, p, u32, p, p, p]
         lib.hough_vote_peaks.argtypes = [p, u32, p, u64, p, p, p, u32, p, p, p]
         lib.hough_jets.argtypes = [p, u32, p, p, f32, f32, u32, p, p, p, p, p]
+        lib.hough_jets_static.argtypes = [C.POINTER(HoughConfig), u32, p, p, f32, f32, u32, p, p, p, p, p]
         lib.hough_trigger_host.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, p, p, p, p, p, p, p]
         lib.hough_trigger_host_vtx.argtypes = [p, u32, p, u64, p, p, p, u32, f32, f32, u32, u32, p, p, p, p, p, p, p, p, p, p]
         lib.hough_vertices.argtypes = [p, u32, p, p, f32, u32, p, p, p, p, p]
@@ -119,6 +121,19 @@ def _stream_ptr(stream=None) -> C.c_void_p:
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
     return C.c_void_p(s.cuda_stream)
+
+
+def hough_jets_static(cfg: HoughConfig, n_events, d_peaks, d_n_peaks, cone_rad, d0_cut_mm, n_displaced_min, d_tracks,
+                      d_jets, d_n_jets, d_flag, stream=None):
+    """hough_jets for callers that may not allocate device memory (a process on a fixed memory budget, a real-time
+    loop, a plug-in whose host owns the allocator): no context, hence no hough_create and no cudaMalloc.  `cfg` is a
+    HoughConfig describing the grid (host side); the tensors are the caller's device buffers as for Hough.hough_jets.
+    The scratch is a fixed array inside the library: HoughError(ETOOLARGE) if n_events * max_peaks_per_event >
+    JETS_STATIC_MAX_TRACKS or n_d0 > JETS_STATIC_MAX_D0.  All calls on a device share that array, so keep them
+    ordered on the GPU (one stream, or events between streams)."""
+    _check(load_library().hough_jets_static(C.byref(cfg), n_events, _dptr(d_peaks), _dptr(d_n_peaks), cone_rad,
+                                            d0_cut_mm, n_displaced_min, _dptr(d_tracks), _dptr(d_jets),
+                                            _dptr(d_n_jets), _dptr(d_flag), _stream_ptr(stream)), "hough_jets_static")
 
 
 class Hough:

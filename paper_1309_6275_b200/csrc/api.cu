@@ -106,6 +106,9 @@ const char* hough_strerror(int code)
         case HOUGH_ECUDA: return g_errbuf[0] ? g_errbuf : "CUDA runtime error";
         case HOUGH_ENOMEM: return "device allocation failed";
         case HOUGH_EUNSUPPORTED: return "configuration not supported by the kernels";
+        case HOUGH_ETOOLARGE:
+            return "hough_jets_static: n_events * max_peaks_per_event exceeds HOUGH_JETS_STATIC_MAX_TRACKS or n_d0 exceeds "
+                   "HOUGH_JETS_STATIC_MAX_D0 (the scratch array is fixed; create a context and use hough_jets instead)";
     }
     return "unknown error code";
 }
@@ -368,6 +371,30 @@ int hough_jets(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, con
     CK(launch_jets(ctx, n_events, d_peaks, d_n_peaks, cone_bins_of(cone_rad, ctx->cfg.n_phi0), d0_cut_mm,
                    n_displaced_min, d_tracks, d_jets, d_n_jets, d_flag, st), "jet kernel");
     prof_mark(ctx, -1, st);
+    return HOUGH_OK;
+}
+
+// hough_jets for callers that may not allocate (no context, no cudaMalloc): see include/hough.h and jets.cu.
+int hough_jets_static(const hough_config* cfg, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
+                      float cone_rad, float d0_cut_mm, uint32_t n_displaced_min, hough_track* d_tracks, hough_jet* d_jets,
+                      uint32_t* d_n_jets, uint8_t* d_flag, void* stream)
+{
+    if (!cfg || !d_peaks || !d_n_peaks || !d_tracks || !d_jets || !d_n_jets || !d_flag) return HOUGH_EINVAL;
+    // the fields the jet kernel reads, with hough_create's conditions on them
+    if (cfg->n_phi0 < 4 || cfg->n_phi0 > (1u << 20)) return HOUGH_EINVAL;
+    if (cfg->n_kappa < 8 || cfg->n_kappa % 8 != 0 || cfg->n_kappa > (1u << 20)) return HOUGH_EINVAL;
+    if (cfg->n_d0 < 1 || cfg->n_d0 > (1u << 16)) return HOUGH_EINVAL;
+    if ((uint64_t)cfg->n_phi0 * cfg->n_kappa * cfg->n_d0 > 0xffffffffull) return HOUGH_EINVAL;
+    if (!(cfg->kappa_max > 0.f) || !isfinite(cfg->kappa_max) || !isfinite(cfg->b_tesla)) return HOUGH_EINVAL;
+    if (cfg->n_d0 > 1 && !(cfg->d0_max > cfg->d0_min && isfinite(cfg->d0_min) && isfinite(cfg->d0_max))) return HOUGH_EINVAL;
+    if (cfg->max_peaks_per_event < 1 || cfg->max_jets_per_event < 1) return HOUGH_EINVAL;
+    if (!(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm)) return HOUGH_EINVAL;
+    // the scratch is a fixed array: refuse what does not fit instead of writing past it
+    if (cfg->n_d0 > HOUGH_JETS_STATIC_MAX_D0) return HOUGH_ETOOLARGE;
+    if ((uint64_t)n_events * cfg->max_peaks_per_event > (uint64_t)HOUGH_JETS_STATIC_MAX_TRACKS) return HOUGH_ETOOLARGE;
+    CK(launch_jets_static(cfg, n_events, d_peaks, d_n_peaks, cone_bins_of(cone_rad, cfg->n_phi0), d0_cut_mm,
+                          n_displaced_min, d_tracks, d_jets, d_n_jets, d_flag, (cudaStream_t)stream),
+       "hough_jets_static (scratch address look-up or kernel launch)");
     return HOUGH_OK;
 }
 

@@ -119,6 +119,11 @@ cudaError_t launch_peaks(hough_ctx* c, uint32_t n_events, const uint16_t* d_coun
 cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
                         int cone_bins, float d0_cut, uint32_t n_min, hough_track* d_tracks, hough_jet* d_jets,
                         uint32_t* d_n_jets, uint8_t* d_flag, cudaStream_t st);
+// hough_jets_static: no context; scratch in the library's own static device array (jets.cu)
+cudaError_t launch_jets_static(const hough_config* g, uint32_t n_events, const hough_peak* d_peaks,
+                               const uint32_t* d_n_peaks, int cone_bins, float d0_cut, uint32_t n_min,
+                               hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag,
+                               cudaStream_t st);
 cudaError_t launch_vote_fused(hough_ctx* c, uint32_t first_event, uint32_t n_events, uint32_t l_min, cudaStream_t st);
 cudaError_t launch_recount(hough_ctx* c, uint32_t first_event, uint32_t n_events, cudaStream_t st);
 cudaError_t launch_peaks_finalize(hough_ctx* c, uint32_t n_events, hough_peak* d_peaks, uint32_t* d_n_peaks,

@@ -4,6 +4,8 @@
 // DESIGN.md O-4 / O-5 (PAPER.md:87 transverse-momentum measurement; PAPER.md:113-123 jets and the
 // interaction-point remark; clustering rule from north_star as read in R17-R22).  All decisions are taken on
 // integer bin keys; floats only appear in the reported fields (tolerance 1e-5).
+#include <mutex>
+
 #include "hough_internal.cuh"
 
 namespace {
@@ -162,5 +164,91 @@ cudaError_t launch_jets(hough_ctx* c, uint32_t n_events, const hough_peak* d_pea
     if (n_events < 64) jets_kernel<8><<<n_events, 256, 0, st>>>(p);
     else jets_kernel<1><<<n_events, 32, 0, st>>>(p);
     ++c->launches;
+    return cudaGetLastError();
+}
+
+// ---- hough_jets_static: the same kernel for callers that may not allocate ---------------------------------------
+//
+// Some users of this library cannot create a context because hough_create calls cudaMalloc: a trigger process whose
+// device memory was all handed out at start-up, a real-time loop that cannot afford the device-wide stall of an
+// allocation, a plug-in whose host runtime owns the allocator.  For them the two pieces of global scratch that
+// jets_kernel needs live in the array below, which is part of this library's device image: it exists on every GPU
+// that loads the library, from module load to process exit, and nobody has to allocate or free it.
+//
+// Layout: [0, kStaticD0Words) the d0 bin centres (float, written by static_d0_table_kernel at every call),
+// then HOUGH_JETS_STATIC_MAX_TRACKS clustering keys (the kernel uses them for events with more than kSmemKeys tracks;
+// it writes key j of an event before any thread reads it, so nothing has to be cleared between calls).
+// All calls on a device share the array: calls that overlap on the GPU race.
+namespace {
+
+constexpr size_t kStaticD0Words = HOUGH_JETS_STATIC_MAX_D0 / 2;                        // uint64 words holding the floats
+constexpr size_t kStaticWords = kStaticD0Words + (size_t)HOUGH_JETS_STATIC_MAX_TRACKS;
+static __device__ __align__(256) unsigned long long g_jets_static_scratch[kStaticWords];
+
+// In host code `g_jets_static_scratch` is only the host-side handle of the symbol, not a device address; the address
+// a kernel can use comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kMaxStaticDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_addr[kMaxStaticDevices] = {};
+
+cudaError_t static_scratch_of_current_device(void** out)
+{
+    int dev = -1;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return err;
+    if (dev < 0 || dev >= kMaxStaticDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        int major = 0;
+        err = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (err != cudaSuccess) return err;
+        if (major < 10) return cudaErrorNoKernelImageForDevice;      // the library holds sm_100a code only
+        void* p = nullptr;
+        err = cudaGetSymbolAddress(&p, g_jets_static_scratch);
+        if (err != cudaSuccess) return err;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_static_addr[dev] = p;
+    }
+    *out = g_static_addr[dev];
+    return cudaSuccess;
+}
+
+// d0 bin centres exactly as hough_create forms them on the host (O-0: double arithmetic, one operation per step,
+// rounded once to fp32); the *_rn intrinsics keep the compiler from contracting the multiply and the add
+__global__ void static_d0_table_kernel(float* d0c, uint32_t nd, double d0_min, double d0_max)
+{
+    const uint32_t id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= nd) return;
+    const double w = __ddiv_rn(__dsub_rn(d0_max, d0_min), (double)nd);
+    d0c[id] = __double2float_rn(__dadd_rn(d0_min, __dmul_rn((double)id + 0.5, w)));
+}
+
+}  // namespace
+
+cudaError_t launch_jets_static(const hough_config* g, uint32_t n_events, const hough_peak* d_peaks,
+                               const uint32_t* d_n_peaks, int cone_bins, float d0_cut, uint32_t n_min,
+                               hough_track* d_tracks, hough_jet* d_jets, uint32_t* d_n_jets, uint8_t* d_flag,
+                               cudaStream_t st)
+{
+    void* base = nullptr;
+    cudaError_t err = static_scratch_of_current_device(&base);
+    if (err != cudaSuccess) return err;
+    if (n_events == 0) return cudaSuccess;
+    float* d0c = reinterpret_cast<float*>(base);
+    if (g->n_d0 > 1) {
+        static_d0_table_kernel<<<(g->n_d0 + 255) / 256, 256, 0, st>>>(d0c, g->n_d0, (double)g->d0_min, (double)g->d0_max);
+        err = cudaGetLastError();
+        if (err != cudaSuccess) return err;
+    }
+    JetParams p;
+    p.peaks = d_peaks; p.n_peaks = d_n_peaks; p.tracks = d_tracks; p.jets = d_jets; p.n_jets = d_n_jets;
+    p.flag = d_flag;
+    p.keys = reinterpret_cast<uint64_t*>(base) + kStaticD0Words;
+    p.d0c = d0c;
+    p.n_events = n_events; p.max_peaks = g->max_peaks_per_event; p.max_jets = g->max_jets_per_event;
+    p.n_d0 = (int)g->n_d0; p.n_phi0 = (int)g->n_phi0; p.n_kappa = (int)g->n_kappa;
+    p.kmax = g->kappa_max; p.b_tesla = g->b_tesla; p.d0_cut = d0_cut; p.cone_bins = cone_bins; p.n_min = n_min;
+    if (n_events < 64) jets_kernel<8><<<n_events, 256, 0, st>>>(p);
+    else jets_kernel<1><<<n_events, 32, 0, st>>>(p);
     return cudaGetLastError();
 }
