@@ -54,12 +54,22 @@ typedef struct {
     uint32_t n_vtx_r;              /* R_v bins over [vtx_r_min, vtx_r_max), half-open; multiple of 8, >= 8;
                                       n_vtx_phi * n_vtx_r * 2 bytes must fit in shared memory (<= 200 KB)            */
     float    vtx_r_min, vtx_r_max; /* mm; vtx_r_min = radius inside which vertices are dropped (beam pipe, 30 mm)     */
-    uint32_t max_vertices_per_event;
+    uint32_t max_vertices_per_event; /* with a vertex grid, max_peaks_per_event must be <= 65535 (16-bit vertex counts)  */
     uint32_t vote_flags;           /* physics-quality voting variants (O-2h / O-2f), accumulator
                                       path only: HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL; 0 = the normative one-vote-per-column-
                                       centre rule of north_star.  hough_vote_peaks / hough_trigger_host* return
                                       HOUGH_EUNSUPPORTED when it is not 0                                             */
+    uint32_t debug_flags;          /* HOUGH_DEBUG_*: which kernel variant runs where the library would choose by itself.
+                                      For tests and measurements; 0 in production.  They change speed, never results.
+                                      (The library reads no environment variable and keeps no state outside a context,
+                                      SURVEY.md section 5.)                                                             */
 } hough_config;
+
+enum {
+    HOUGH_DEBUG_NO_MIRROR = 1u,    /* plain tiles also on grids whose tables allow mirror tiles (hence no mask tiles)   */
+    HOUGH_DEBUG_TILES_COUNT = 2u,  /* hough_vote_peaks: always count + mask tiles                                       */
+    HOUGH_DEBUG_TILES_MASK = 4u    /* hough_vote_peaks: mask tiles whenever the grid has them (not both TILES bits)     */
+};
 
 enum {
     HOUGH_VOTE_HEMI = 1u,   /* forward-hemisphere cut: a (hit, column) votes only if cos(phi - phi0c) > 0 (no mirror peaks) */
@@ -151,8 +161,8 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
  * tiles" accumulate both, compare a candidate with its neighbours inside the tile and have only the neighbours
  * across a tile border recomputed.  A call starts with mask tiles when the grid allows them (mirror-symmetric
  * tables) and few chance candidates are expected, and votes the events whose candidates overflow the buffer again
- * with count + mask tiles, on the device; the result does not depend on the kind of tile (environment variable
- * HOUGH_FUSED_TILES=mask|count, read by hough_create, forces one: tests).
+ * with count + mask tiles, on the device; the result does not depend on the kind of tile (hough_config.debug_flags
+ * HOUGH_DEBUG_TILES_MASK / HOUGH_DEBUG_TILES_COUNT force one: tests).
  *   arguments as hough_vote / hough_peaks.  Capacity: if an event has more than max_candidates_per_event
  *   candidates (count + mask tiles), HOUGH_ST_CANDIDATE_OVERFLOW is raised and d_n_peaks[e] =
  *   HOUGH_N_PEAKS_OVERFLOW (no record of that event is valid; hough_jets treats it as an event without tracks):
@@ -232,9 +242,12 @@ int hough_jets_static(const hough_config* cfg, uint32_t n_events, const hough_pe
  *   d_vertices   [n_events][max_vertices_per_event]; d_n_vertices [n_events] u32 TRUE total; d_flag [n_events] u8
  *   = 1 iff the event has a vertex;  d_vertex_plane: optional (may be null) [n_events][n_vtx_phi][n_vtx_r] u16,
  *   receives the vote counts (tests).
- * n_min in [1, 65535] (the oracle's peak-finder reuse covers 1..16).  HOUGH_EINVAL if the context was created
- * without a vertex grid.
+ * n_min in [1, HOUGH_VTX_N_MIN_MAX]: the range over which the result is checked against the oracle (its reuse of the
+ * peak finder, "the same peak finding algorithm", covers thresholds up to 16); HOUGH_EINVAL outside it, and
+ * if the context was created without a vertex grid.  Counts are 16-bit: a context with a vertex grid must have
+ * max_peaks_per_event <= 65535 (hough_create rejects more), so no bin can receive more votes than it can hold.
  */
+#define HOUGH_VTX_N_MIN_MAX 16u
 int hough_vertices(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks, const uint32_t* d_n_peaks,
                    float d0_cut_mm, uint32_t n_min, hough_vertex* d_vertices, uint32_t* d_n_vertices, uint8_t* d_flag,
                    uint16_t* d_vertex_plane, void* stream);
@@ -247,7 +260,12 @@ int hough_vertices(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks,
  * so the results are always those of the definition.  All h_* pointers are HOST memory (pinned memory makes the
  * copies asynchronous); synchronises `stream` before returning.
  * ms_stage (HOST, may be null) receives the device time in ms spent in {vote (incl. candidate scan), peaks
- * (recount + ordering), jets}.
+ * (recount + ordering), jets}, the fallback's launches included.  A call with ms_stage uses the context's stage
+ * profile: it starts from an empty profile (intervals accumulated with hough_profile and not yet read are dropped)
+ * and leaves hough_profile's on / off setting as it found it, also when it returns an error.
+ * Status: the overflow is repaired inside the call, so the call clears HOUGH_ST_CANDIDATE_OVERFLOW on the device
+ * after the last fallback (a bit raised by an earlier hough_vote_peaks on this context and not yet read by
+ * hough_status goes with it); the other status bits are untouched.
  */
 int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
                        const float* h_r, const float* h_phi, const uint8_t* h_layer,
@@ -260,6 +278,7 @@ int hough_trigger_host(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_
 /*
  * The same with the second Hough transform run after the jets (context created with a vertex grid):
  * h_n_vertices [n_events] u32, h_vtx_flag [n_events] u8, h_vertices [n_events][max_vertices] or null.
+ * vtx_n_min = 0 skips the second transform; otherwise it is hough_vertices' n_min (1..HOUGH_VTX_N_MIN_MAX).
  * ms_stage, if not null, has FOUR entries: {vote, peaks, jets, vertices}.
  */
 int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_hit_offsets, uint64_t n_hits_total,
@@ -283,6 +302,15 @@ int hough_status(hough_ctx* ctx, uint32_t* host_status_bits);
  */
 int hough_profile(hough_ctx* ctx, int enable);
 int hough_profile_read(hough_ctx* ctx, float* h_ms /* [5] */, uint32_t* h_calls /* may be null */);
+
+/*
+ * Which kind of tile the last fused launch on ctx (hough_vote_peaks, or the last chunk of hough_trigger_host*) STARTED
+ * with -- the library's own speed heuristic unless debug_flags forces one: 0 = no fused launch yet,
+ * 1 = count + mask tiles (two shared reductions per vote), 2 = mask tiles (one shared reduction per vote; events whose
+ * candidates overflowed were voted again with count + mask tiles).  The result never depends on it; bench.py uses it to
+ * charge the right number of shared reductions in the roofline.  HOST out.
+ */
+int hough_last_tile_kind(const hough_ctx* ctx, int* host_kind);
 
 /* Number of kernel launches this context has enqueued since creation (bench.py's gpu_launches).  HOST out. */
 int hough_launch_count(const hough_ctx* ctx, uint64_t* host_count);

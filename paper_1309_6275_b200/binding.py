@@ -26,9 +26,10 @@ ST_EVENT_TOO_LARGE, ST_BAD_OFFSETS, ST_TRIG_ROUNDING, ST_CANDIDATE_OVERFLOW = 1,
 ST_ERRORS = ST_EVENT_TOO_LARGE | ST_BAD_OFFSETS            # the bits that mean "results undefined"
 N_PEAKS_OVERFLOW = 0xFFFFFFFF
 VOTE_HEMI, VOTE_FILL = 1, 2
+DEBUG_NO_MIRROR, DEBUG_TILES_COUNT, DEBUG_TILES_MASK = 1, 2, 4      # hough_config.debug_flags (tests, measurements)
 EXPORTS = ["hough_create", "hough_destroy", "hough_plane_bytes", "hough_vote", "hough_peaks", "hough_vote_peaks",
            "hough_jets", "hough_jets_static", "hough_vertices", "hough_trigger_host_vtx",
-           "hough_trigger_host", "hough_status", "hough_launch_count", "hough_microbench", "hough_strerror",
+           "hough_trigger_host", "hough_status", "hough_launch_count", "hough_last_tile_kind", "hough_microbench", "hough_strerror",
            "hough_debug_prepared_hits", "hough_debug_div_check", "hough_profile", "hough_profile_read"]
 
 
@@ -39,7 +40,7 @@ class HoughConfig(C.Structure):
                 ("max_peaks_per_event", C.c_uint32), ("max_jets_per_event", C.c_uint32),
                 ("host_chunk_events", C.c_uint32), ("max_candidates_per_event", C.c_uint32),
                 ("n_vtx_phi", C.c_uint32), ("n_vtx_r", C.c_uint32), ("vtx_r_min", C.c_float), ("vtx_r_max", C.c_float),
-                ("max_vertices_per_event", C.c_uint32), ("vote_flags", C.c_uint32)]
+                ("max_vertices_per_event", C.c_uint32), ("vote_flags", C.c_uint32), ("debug_flags", C.c_uint32)]
 
 
 class HoughError(RuntimeError):
@@ -75,6 +76,7 @@ def load_library() -> C.CDLL:
         lib.hough_vertices.argtypes = [p, u32, p, p, f32, u32, p, p, p, p, p]
         lib.hough_status.argtypes = [p, C.POINTER(u32)]
         lib.hough_launch_count.argtypes = [p, C.POINTER(u64)]
+        lib.hough_last_tile_kind.argtypes = [p, C.POINTER(C.c_int)]
         lib.hough_microbench.argtypes = [C.c_int, C.c_size_t, C.POINTER(C.c_double)]
         lib.hough_debug_prepared_hits.argtypes = [p, u64, p, C.POINTER(u32)]
         lib.hough_debug_div_check.argtypes = [u64, u64, f32, u32, C.POINTER(u64)]
@@ -144,19 +146,20 @@ class Hough:
                  max_events: int = 1, max_hits: int = 1 << 16, max_peaks_per_event: int = 4096,
                  max_jets_per_event: int = 256, host_chunk_events: int = 0, max_candidates_per_event: int = 0,
                  n_vtx_phi: int = 0, n_vtx_r: int = 0, vtx_r_min: float = 30.0, vtx_r_max: float = 430.0,
-                 max_vertices_per_event: int = 64, vote_flags: int = 0):
+                 max_vertices_per_event: int = 64, vote_flags: int = 0, debug_flags: int = 0):
         self.lib = load_library()
         self.cfg = HoughConfig(n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, n_layers, max_events,
                                max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events,
                                max_candidates_per_event, n_vtx_phi, n_vtx_r, vtx_r_min, vtx_r_max,
-                               max_vertices_per_event, vote_flags)
+                               max_vertices_per_event, vote_flags, debug_flags)
         self._ctx = C.c_void_p()
         _check(self.lib.hough_create(C.byref(self.cfg), C.byref(self._ctx)), "hough_create")
 
     @classmethod
     def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
                      host_chunk_events: int = 0, max_peaks: Optional[int] = None,
-                     max_candidates: int = 0, vgrid=None, max_vertices: int = 64, vote_flags: int = 0) -> "Hough":
+                     max_candidates: int = 0, vgrid=None, max_vertices: int = 64, vote_flags: int = 0,
+                     debug_flags: int = 0) -> "Hough":
         """vgrid: None, or (n_vtx_phi, n_vtx_r, r_min, r_max) for the second Hough transform (hough_vertices)."""
         ne = w.n_events if max_events is None else max_events
         if max_hits is None:
@@ -165,7 +168,8 @@ class Hough:
         mh = max_hits
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
                    min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
-                   host_chunk_events, max_candidates, *((0, 0, 30.0, 430.0) if vgrid is None else vgrid), max_vertices, vote_flags)
+                   host_chunk_events, max_candidates, *((0, 0, 30.0, 430.0) if vgrid is None else vgrid), max_vertices, vote_flags,
+                   debug_flags)
 
     # -- lifetime ---------------------------------------------------------------------------------
     def close(self):
@@ -286,6 +290,12 @@ class Hough:
         ms = (C.c_float * 5)(); n = C.c_uint32(0)
         _check(self.lib.hough_profile_read(self._ctx, ms, C.byref(n)), "hough_profile_read")
         return [float(x) for x in ms], int(n.value)
+
+    def hough_last_tile_kind(self) -> int:
+        """0 no fused launch yet, 1 count + mask tiles, 2 mask tiles (what the last fused launch started with)."""
+        out = C.c_int(0)
+        _check(self.lib.hough_last_tile_kind(self._ctx, C.byref(out)), "hough_last_tile_kind")
+        return out.value
 
     def hough_launch_count(self) -> int:
         out = C.c_uint64(0)

@@ -83,6 +83,8 @@ bool config_ok(const hough_config* g)
     if (g->host_chunk_events > g->max_events) return false;
     if (g->max_candidates_per_event > (1u << 24)) return false;
     if (g->vote_flags & ~(uint32_t)(HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL)) return false;
+    if (g->debug_flags & ~(uint32_t)(HOUGH_DEBUG_NO_MIRROR | HOUGH_DEBUG_TILES_COUNT | HOUGH_DEBUG_TILES_MASK)) return false;
+    if ((g->debug_flags & HOUGH_DEBUG_TILES_COUNT) && (g->debug_flags & HOUGH_DEBUG_TILES_MASK)) return false;
     if (g->n_vtx_phi != 0) {                                   // vertex grid of the second transform
         if (g->n_vtx_phi < 8 || g->n_vtx_phi % 4 != 0 || g->n_vtx_r < 8 || g->n_vtx_r % 8 != 0) return false;
         if ((uint64_t)g->n_vtx_phi * g->n_vtx_r * 2 > 200u * 1024u) return false;
@@ -90,9 +92,15 @@ bool config_ok(const hough_config* g)
                 (uint64_t)g->n_vtx_phi * g->n_vtx_r / 8 > 220u * 1024u) return false;
         if (!(g->vtx_r_min > 0.f) || !(g->vtx_r_max > g->vtx_r_min) || !isfinite(g->vtx_r_max)) return false;
         if (g->max_vertices_per_event < 1) return false;
+        // every stored track votes at most once per R_v bin and the vertex plane counts in 16 bits (two counts per
+        // 32-bit word, vertices.cu): more than 65535 tracks could carry from one bin into its neighbour
+        if (g->max_peaks_per_event > 65535u) return false;
     }
     return true;
 }
+
+// hough_trigger_host: takes sticky status bits back once the condition they report has been repaired
+__global__ void status_clear_kernel(uint32_t* status, uint32_t bits) { atomicAnd(status, ~bits); }
 
 }  // namespace
 
@@ -168,15 +176,14 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
         const double a = (double)j * (2.0 * pi / (double)NP);
         ce[j] = (float)cos(a); se[j] = (float)sin(a);
     }
-    bool mirror_ok = NP % 2 == 0 && getenv("HOUGH_NO_MIRROR") == nullptr && cfg->vote_flags == 0;
+    bool mirror_ok = NP % 2 == 0 && !(cfg->debug_flags & HOUGH_DEBUG_NO_MIRROR) && cfg->vote_flags == 0;
     for (uint32_t ip = 0; mirror_ok && ip < NP / 2; ++ip)
         mirror_ok = c0[ip + NP / 2] == -c0[ip] && s0[ip + NP / 2] == -s0[ip];
     for (uint32_t id = 0; mirror_ok && id < ND; ++id) mirror_ok = d0c[ND - 1 - id] == -d0c[id];
     if (plan_vote(c, mirror_ok) != cudaSuccess || plan_peaks(c) != cudaSuccess) { delete c; return HOUGH_EUNSUPPORTED; }
-    // fused path: which tiles hough_vote_peaks uses on a grid that has both kinds (debug / test switch, read once):
-    // HOUGH_FUSED_TILES=count -> count + mask tiles, =mask -> mask-only tiles, unset -> chosen per call by occupancy
-    c->fused_scheme = 0;
-    if (const char* ft = getenv("HOUGH_FUSED_TILES")) c->fused_scheme = (ft[0] == 'c') ? 1 : (ft[0] == 'm') ? 2 : 0;
+    // fused path: which tiles hough_vote_peaks uses on a grid that has both kinds: cfg.debug_flags can force
+    // count + mask tiles (1) or mask-only tiles (2); otherwise (0) chosen per call by occupancy
+    c->fused_scheme = (cfg->debug_flags & HOUGH_DEBUG_TILES_COUNT) ? 1 : (cfg->debug_flags & HOUGH_DEBUG_TILES_MASK) ? 2 : 0;
     c->prep_hits_per_event = 0.0;
     // the branch-free exact division of the vote kernel is only used inside this range (vote.cu, div_rn_tame)
     c->tame_tables = cfg->kappa_max >= 9.094947e-13f && cfg->kappa_max <= 1.0995116e12f;      // [2^-40, 2^40]
@@ -403,7 +410,7 @@ int hough_vertices(hough_ctx* ctx, uint32_t n_events, const hough_peak* d_peaks,
                    uint16_t* d_vertex_plane, void* stream)
 {
     if (!ctx || !d_peaks || !d_n_peaks || !d_vertices || !d_n_vertices || !d_flag) return HOUGH_EINVAL;
-    if (ctx->cfg.n_vtx_phi == 0 || n_events > ctx->cfg.max_events || n_min < 1 || n_min > 65535u || isnan(d0_cut_mm))
+    if (ctx->cfg.n_vtx_phi == 0 || n_events > ctx->cfg.max_events || n_min < 1 || n_min > HOUGH_VTX_N_MIN_MAX || isnan(d0_cut_mm))
         return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
@@ -429,7 +436,7 @@ int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_
     if (l_min < 1 || l_min > ctx->cfg.n_layers || !(cone_rad >= 0.f) || !isfinite(cone_rad) || isnan(d0_cut_mm))
         return HOUGH_EINVAL;
     const bool vtx = vtx_n_min != 0;                            // 0: the second transform is not run
-    if (vtx && (ctx->cfg.n_vtx_phi == 0 || vtx_n_min > 65535u || !h_n_vertices || !h_vtx_flag)) return HOUGH_EINVAL;
+    if (vtx && (ctx->cfg.n_vtx_phi == 0 || vtx_n_min > HOUGH_VTX_N_MIN_MAX || !h_n_vertices || !h_vtx_flag)) return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;
     const int n_stage = vtx ? 4 : 3;
@@ -443,10 +450,16 @@ int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_
         CK(cudaMemcpyAsync(ctx->d_hp_layer, h_layer, n_hits_total, cudaMemcpyHostToDevice, st), "H2D layer");
     }
     // ms_stage: the context's stage profile (hough_profile) is switched on for this call and read at its end
-    const bool prof_was_on = ctx->prof_on;
+    // (documented in hough.h: a call with ms_stage starts from an empty profile, so intervals the caller had
+    // accumulated with hough_profile and not yet read are dropped -- as are marks left behind by a profile that was
+    // switched off without a read).  The guard puts the caller's setting back on EVERY way out, error returns included.
+    struct ProfRestore {
+        hough_ctx* c; bool was_on; bool armed;
+        ~ProfRestore() { if (armed) c->prof_on = was_on; }
+    } prof_restore{ctx, ctx->prof_on, ms_stage != nullptr};
     if (ms_stage) {
         float drop[5]; uint32_t nc = 0;
-        if (prof_was_on) hough_profile_read(ctx, drop, &nc);     // keep earlier intervals out of this call's numbers
+        hough_profile_read(ctx, drop, &nc);                      // empties the mark list whatever state it was in
         ctx->prof_on = true;
     }
     auto peaks_of = [&](uint32_t e) { return ctx->d_hp_peaks + (size_t)e * g.max_peaks_per_event; };
@@ -480,14 +493,25 @@ int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_
     CK(cudaStreamSynchronize(st), "hough_trigger_host synchronize");
     // events whose candidates did not fit the buffer: the accumulator path, one event at a time, on the context's
     // one-event planes (the prepared hits of the whole batch are still in the workspace)
+    uint32_t n_repaired = 0;
     for (uint32_t e = 0; e < n_events; ++e) {
         if (h_n_peaks[e] != HOUGH_N_PEAKS_OVERFLOW) continue;
+        prof_mark(ctx, 1, st);                                   // the fallback's time belongs to ms_stage as well
         CK(launch_vote(ctx, e, 1, ctx->d_hp_count, ctx->d_hp_mask, st), "vote kernel (fallback)");
+        prof_mark(ctx, 2, st);
         CK(launch_peaks(ctx, 1, ctx->d_hp_count, ctx->d_hp_mask, l_min, peaks_of(e), ctx->d_hp_npeaks + e, st),
            "peak kernels (fallback)");
         CK(tail(e, 1, cone_bins), "jet / vertex kernels (fallback)");
         prof_mark(ctx, -1, st);
         CK(cudaMemcpyAsync(h_n_peaks + e, ctx->d_hp_npeaks + e, 4, cudaMemcpyDeviceToHost, st), "D2H n_peaks (fallback)");
+        ++n_repaired;
+    }
+    if (n_repaired) {
+        // every overflowed event now holds the accumulator path's (exact) result: the overflow bit this call raised
+        // would report an error that no longer exists
+        status_clear_kernel<<<1, 1, 0, st>>>(ctx->d_status, (uint32_t)HOUGH_ST_CANDIDATE_OVERFLOW);
+        ++ctx->launches;
+        CK(cudaGetLastError(), "status kernel");
     }
     CK(cudaMemcpyAsync(h_n_jets, ctx->d_hp_njets, (size_t)n_events * 4, cudaMemcpyDeviceToHost, st), "D2H n_jets");
     CK(cudaMemcpyAsync(h_flag, ctx->d_hp_flag, (size_t)n_events, cudaMemcpyDeviceToHost, st), "D2H flag");
@@ -510,7 +534,6 @@ int hough_trigger_host_vtx(hough_ctx* ctx, uint32_t n_events, const uint32_t* h_
         hough_profile_read(ctx, ms, &nc);
         ms_stage[0] = ms[0] + ms[1]; ms_stage[1] = ms[2]; ms_stage[2] = ms[3];
         if (vtx) ms_stage[3] = ms[4];
-        ctx->prof_on = prof_was_on;
     }
     return HOUGH_OK;
 }
@@ -580,6 +603,13 @@ int hough_profile_read(hough_ctx* ctx, float* h_ms, uint32_t* h_calls)
     if (ctx->ev_used) ++calls;
     ctx->ev_used = 0;
     if (h_calls) *h_calls = calls;
+    return HOUGH_OK;
+}
+
+int hough_last_tile_kind(const hough_ctx* ctx, int* host_kind)
+{
+    if (!ctx || !host_kind) return HOUGH_EINVAL;
+    *host_kind = ctx->last_tile_kind;
     return HOUGH_OK;
 }
 

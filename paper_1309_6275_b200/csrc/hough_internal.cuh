@@ -87,7 +87,7 @@ struct hough_ctx {
     uint32_t* d_cand_n;                       // [fused_events], zero between calls
     unsigned long long* d_sortkeys;           // [fused_events][cand_cap_pow2] sort scratch for events beyond the SMEM sort
     // host path
-    uint16_t* d_hp_count; uint16_t* d_hp_mask;     // [host_chunk_events][bins]
+    uint16_t* d_hp_count; uint16_t* d_hp_mask;     // [bins]: the planes of ONE event (fallback of hough_trigger_host)
     uint32_t* d_hp_off; float* d_hp_r; float* d_hp_phi; uint8_t* d_hp_layer;
     hough_peak* d_hp_peaks; hough_track* d_hp_tracks; hough_jet* d_hp_jets;
     uint32_t* d_hp_npeaks; uint32_t* d_hp_njets; uint8_t* d_hp_flag;
@@ -100,7 +100,8 @@ struct hough_ctx {
     VotePlan vote;
     VotePlan vote_mo;                         // fused path, mask-only mirror tiles (has_mo): larger kappa range per tile
     bool has_mo;
-    int fused_scheme;                         // 0: choose per call by occupancy, 1: count + mask tiles, 2: mask tiles (HOUGH_FUSED_TILES)
+    int fused_scheme;                         // 0: choose per call by occupancy, 1: count + mask tiles, 2: mask tiles (cfg.debug_flags)
+    int last_tile_kind;                       // tiles the last fused launch started with: 0 none yet, 1 count + mask, 2 mask (hough_last_tile_kind)
     double prep_hits_per_event;               // mean hits per event of the last launch_prep (tile choice of the fused path)
     uint32_t* d_redo;                         // [1 + fused_events]: number and indices of the events whose mask-tile candidates overflowed
     PeakPlan peak;

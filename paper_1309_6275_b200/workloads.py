@@ -148,7 +148,7 @@ def paper_efficiency(kind: str, x: int, n_events: int = 64) -> Workload:
     if kind == "F9":
         return Workload(f"F9-{x}", 90, n_prompt=(0, 0), n_llp=(x, x), llp_tracks=(10, 10), **base)
     if kind == "F10":
-        base["max_peaks"] = 65536
+        base["max_peaks"] = 65535                                # the most a context with a vertex grid accepts (hough.h)
         return Workload(f"F10-{x}", 100, n_prompt=(3000 - 10 * x, 3000 - 10 * x), n_llp=(x, x), llp_tracks=(10, 10), **base)
     raise ValueError("kind must be F8, F9 or F10")
 

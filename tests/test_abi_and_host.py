@@ -42,6 +42,9 @@ def test_strerror_and_argument_validation_without_gpu():
     assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
     bad2 = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 17, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0)     # n_layers > 16
     assert lib.hough_create(C.byref(bad2), C.byref(ctx)) == -1
+    # a vertex grid counts tracks in 16 bits: a peak list that could overflow a bin is refused (hough.h)
+    bad3 = B.HoughConfig(512, 256, 8, 1.14e-3, -10.0, 10.0, 3.8, 8, 1, 100, 65536, 16, 0, 0, 64, 32, 30.0, 430.0, 16, 0)
+    assert lib.hough_create(C.byref(bad3), C.byref(ctx)) == -1
     assert lib.hough_create(None, C.byref(ctx)) == -1
     assert lib.hough_destroy(None) == -1
     assert lib.hough_plane_bytes(None, 3) == 0
@@ -57,10 +60,9 @@ def test_config_struct_layout_matches_header():
     int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(hough_config), offsetof(hough_config, max_hits),
         offsetof(hough_config, host_chunk_events), sizeof(hough_peak), sizeof(hough_track), sizeof(hough_jet),
         offsetof(hough_config, max_events), offsetof(hough_config, max_candidates_per_event));
-        printf("%zu %zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex),
-               offsetof(hough_config, vote_flags));
+        printf("%zu %zu %zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex),
+               offsetof(hough_config, vote_flags), offsetof(hough_config, debug_flags));
         return 0; }'''
-    exe = os.path.join(ROOT, "_work", "layout_probe") if os.path.isdir(os.path.join(ROOT, "_work")) else "/tmp/layout_probe"
     exe = "/tmp/hough_layout_probe"
     subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=src, text=True, check=True)
     vals = list(map(int, subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()))
@@ -69,6 +71,7 @@ def test_config_struct_layout_matches_header():
     assert vals[6] == B.HoughConfig.max_events.offset and vals[7] == B.HoughConfig.max_candidates_per_event.offset
     assert vals[8] == B.HoughConfig.vtx_r_min.offset and vals[9] == B.HoughConfig.max_vertices_per_event.offset
     assert vals[10] == B.VERTEX_DTYPE.itemsize == 16 and vals[11] == B.HoughConfig.vote_flags.offset
+    assert vals[12] == B.HoughConfig.debug_flags.offset
     assert vals[3] == B.PEAK_DTYPE.itemsize == 8 and vals[4] == B.TRACK_DTYPE.itemsize == 20
     assert vals[5] == B.JET_DTYPE.itemsize == 20
 
@@ -103,6 +106,20 @@ def test_packed_sweep_keeps_every_rounding_of_o2():
             assert n_mul == 2 * n_rm, (n_mul, n_rm)
             assert n_fma == 5 * n_rm, (n_fma, n_rm)
     assert n_mirror == 3
+
+
+def test_library_reads_no_environment_variable_and_rejects_unknown_debug_flags():
+    """no environment variables, no global state.  Kernel variants are chosen through
+    hough_config.debug_flags; nothing under csrc/ calls getenv."""
+    from paper_1309_6275_b200 import binding as B
+    csrc = os.path.join(ROOT, "paper_1309_6275_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    lib = B.load_library()
+    ctx = C.c_void_p()
+    for flags in (8, B.DEBUG_TILES_COUNT | B.DEBUG_TILES_MASK):
+        bad = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0, flags)
+        assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
 
 
 def test_product_path_never_touches_the_oracle():
