@@ -169,9 +169,11 @@ def measured_peaks():
 
 
 def traffic_from_profiles(kernel_substr: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum (GB per launch) of the newest committed `ncu --page raw --csv`
-    export under profiles/ whose kernel name contains kernel_substr; (None, None) if there is none."""
-    best = (None, None)
+    """(dram__bytes_read.sum + dram__bytes_write.sum in GB per launch, file name, FMA-pipe busy fraction) of the newest
+    committed `ncu --page raw --csv` export under profiles/ whose kernel name contains kernel_substr; (None, None, None)
+    if there is none.  The pipe fraction is sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed / 100: what
+    the FP32 pipe was measured to do, next to the model-work fraction the roofline reports."""
+    best = (None, None, None)
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_raw.csv"))):
         try:
             rows = list(csv.reader(open(path, newline="")))
@@ -193,7 +195,12 @@ def traffic_from_profiles(kernel_substr: str):
                          float(row[i_w].replace(",", "")) * scale[units[i_w]]
                 except Exception:
                     continue
-                best = (gb, os.path.basename(path))
+                fma = None
+                try:
+                    fma = float(row[head.index("sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed")]) / 100.0
+                except Exception:
+                    pass
+                best = (gb, os.path.basename(path), fma)
     return best
 
 
@@ -339,6 +346,7 @@ class DeviceRun:
         if dist: dist.barrier()
         stage, _ = self.h.hough_profile_read()
         self.h.hough_profile(False)
+        self.tile_kind = self.h.hough_last_tile_kind() if self.path == "fused" else 1
         return a.elapsed_time(b), stage, self.h.hough_launch_count() - l0
 
     def close(self):
@@ -369,16 +377,25 @@ def count_votes(w, batch, sub: int = 16):
     return float(total)
 
 
-def vote_roofline(mode, votes, bins_written, ms_vote, launches, hbm_gbs, sm_max_mhz, peak_src, kernel, traffic=None):
+def vote_roofline(mode, votes, bins_written, ms_vote, launches, hbm_gbs, sm_max_mhz, peak_src, kernel, traffic=None,
+                  tile_kind=1):
     """Roofline of the vote kernel: max of the FP32 term (I_FP32 instructions per vote on 148 x 128 lanes), the
-    shared-reduction term (2 per vote at 32 per clock and SM) and -- accumulator path only -- the HBM-write term
-    (4 B per bin)."""
+    shared-reduction term (count + mask tiles: 2 per vote, mask tiles: 1 per vote, at 32 per clock and SM) and --
+    accumulator path only -- the HBM-write term (4 B per bin).
+
+    What `frac` is when the FP32 term binds: a MODEL-WORK fraction -- landed votes x the FP32 instructions the plain
+    O-2 formulation spends per vote, over time x FP32 issue peak.  It is not the measured utilisation of the pipe: mirror
+    tiles evaluate one O-2 chain for two votes and the packed fp32x2 arithmetic halves the issue count again, so the
+    kernel issues fewer instructions per vote than the model charges and the fraction could exceed 1.  The measured
+    pipe figure of the same kernel, where a committed ncu capture has it, is reported next to it as
+    `fma_pipe_active_ncu`."""
     s = ms_vote * 1e-3
     clk = sm_max_mhz * 1e6
     fp32_peak = SM_COUNT * FP32_LANES * clk
     red_peak = SM_COUNT * SMEM_RED_PER_CLK * clk
+    reds_per_vote = 1.0 if tile_kind == 2 else 2.0
     t_fp32 = votes * I_FP32[mode] / fp32_peak
-    t_red = 2.0 * votes / red_peak
+    t_red = reds_per_vote * votes / red_peak
     t_hbm = 4.0 * bins_written / (hbm_gbs * 1e9)
     terms = {"fp32": t_fp32 * 1e3, "shared_reductions": t_red * 1e3, "hbm_write": t_hbm * 1e3}
     if t_hbm >= max(t_fp32, t_red):
@@ -387,9 +404,14 @@ def vote_roofline(mode, votes, bins_written, ms_vote, launches, hbm_gbs, sm_max_
     else:
         ach = votes * I_FP32[mode] / s
         rl = {"bound": "alu", "achieved": ach / 1e12, "peak": fp32_peak / 1e12, "unit": "Tinstr/s",
-              "frac": ach / fp32_peak}
+              "frac": ach / fp32_peak,
+              "frac_kind": "model work: landed votes x I_FP32 (FP32 instructions per vote of the plain O-2 formulation) "
+                           "/ (vote time x FP32 issue peak); not measured pipe utilisation, can exceed 1 on mirror / "
+                           "packed tiles; evaluated (hit, row) pairs are not counted by the kernel"}
     rl.update({"traffic": traffic[0] if traffic else None, "traffic_source": traffic[1] if traffic else None,
+               "fma_pipe_active_ncu": traffic[2] if traffic else None,
                "kernel": kernel, "ms_per_launch": ms_vote / max(1, launches), "launches": launches,
+               "tiles": {0: None, 1: "count + mask", 2: "mask"}.get(tile_kind), "shared_reductions_per_vote": reds_per_vote,
                "i_fp32_per_vote": I_FP32[mode], "t_bound_terms_ms": terms,
                "frac_fp32_shared_hit_terms": votes * I_FP32_SHARED[mode] / s / fp32_peak,
                "peak_source": peak_src + "; FP32 peak = 148 SM x 128 lanes x sm_max clock (no FMA credit)",
@@ -429,7 +451,8 @@ def measure_config(name: str, hbm_gbs, sm_max_mhz, peak_src, steps: int = 3):
         else:
             bins_w = 0 if path == "fused" else w.bins_per_event * w.n_events * reps
             d["roofline"] = vote_roofline(mode, votes * reps, bins_w, stage[1], n_launch, hbm_gbs, sm_max_mhz, peak_src,
-                                          "vote_kernel<fused>" if path == "fused" else "vote_kernel")
+                                          "vote_kernel<fused>" if path == "fused" else "vote_kernel",
+                                          tile_kind=run.tile_kind)
             if path == "planes":
                 d["roofline_stencil"] = stencil_roofline(w.bins_per_event * w.n_events * reps, stage[2], n_launch, hbm_gbs)
         res[path] = d
@@ -467,7 +490,8 @@ def run_p4(args):
                        "stage_ms_per_event": {k: v / args.steps / E for k, v in zip(STAGES, stage)},
                        "roofline": vote_roofline("2d", votes * args.steps, 0 if path == "fused" else w.bins_per_event * E * args.steps,
                                                  stage[1], args.steps, hbm_gbs, sm_max_mhz, peak_src,
-                                                 "vote_kernel<fused>" if path == "fused" else "vote_kernel")}
+                                                 "vote_kernel<fused>" if path == "fused" else "vote_kernel",
+                                                 tile_kind=run.tile_kind)}
             if path == "fused":
                 d["peaks_per_event"] = float(run.out["n_peaks"].float().mean().item())
                 last = (w, batch, ms, stage, launches, votes)
@@ -703,6 +727,7 @@ def run_ours(args):
     total_events = sum_over_ranks(float(E * args.steps), dist)
     value = total_events / (ms_max * 1e-3)
     n_launch = args.steps * run.n_chunks
+    main_tile_kind = run.tile_kind
     run.close()
     torch.cuda.empty_cache()
 
@@ -728,8 +753,13 @@ def run_ours(args):
         torch.cuda.empty_cache()
 
     # ---- e2e: the same batch through hough_trigger_host with pinned host buffers ----
+    # max_plane_events = 1: this context never runs hough_peaks on a batch (only the one-event overflow fallback), so
+    # it need not hold the peak finder's bitmap for max_events events (C5: 34 GB)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
     h2 = B.Hough.for_workload(w, max_events=E, max_hits=H, host_chunk_events=chunk,
-                              vgrid=w.vgrid if with_vtx else None, max_vertices=w.max_vertices)
+                              vgrid=w.vgrid if with_vtx else None, max_vertices=w.max_vertices, max_plane_events=1)
+    e2e_ctx_bytes = int(free0 - torch.cuda.mem_get_info()[0])
     pin = lambda a: torch.from_numpy(a).pin_memory()
     h_off, h_r, h_phi, h_layer = pin(batch.hit_offsets.view(np.int32)), pin(batch.r), pin(batch.phi), pin(batch.layer)
     h_np = torch.zeros(E, dtype=torch.int32).pin_memory(); h_nj = torch.zeros(E, dtype=torch.int32).pin_memory()
@@ -772,7 +802,7 @@ def run_ours(args):
     kern = "vote_kernel<fused>" if fused else "vote_kernel"
     traffic = traffic_from_profiles("vote_kernel") if (w.name == "C5" and chunk == 128) else None
     roofline = vote_roofline(mode, votes_timed, 0 if fused else bins * E * args.steps, stage[1], n_launch, hbm_gbs,
-                             sm_max_mhz, peak_src, kern, traffic)
+                             sm_max_mhz, peak_src, kern, traffic, tile_kind=main_tile_kind)
 
     per_config = None
     if not args.no_per_config and world == 1 and w.name == "C5" and not args.events:
@@ -805,6 +835,7 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(E * 9 + E * w.max_jets * 20 + (E * 5 + E * w.max_vertices * 16 if with_vtx else 0)),
                 "steps": e2e_steps,
                 "matches_device_path": e2e_ok},
+        "e2e_context_device_bytes": e2e_ctx_bytes,
         "gpu_launches": int(launches), "gpu_launches_e2e": int(h2_launches),
         "roofline": roofline,
     }

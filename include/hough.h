@@ -59,6 +59,11 @@ typedef struct {
                                       path only: HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL; 0 = the normative one-vote-per-column-
                                       centre rule of north_star.  hough_vote_peaks / hough_trigger_host* return
                                       HOUGH_EUNSUPPORTED when it is not 0                                             */
+    uint32_t max_plane_events;     /* accumulator path: events per hough_peaks call the peak finder's scratch is sized for
+                                      (per event: 1 bit per bin + 2 B per 256 bins); 0 = max_events.  hough_peaks returns
+                                      HOUGH_EINVAL beyond it.  A context that is only used through hough_vote_peaks /
+                                      hough_trigger_host* can set 1 (the host path's overflow fallback needs one event): on
+                                      C5 that is 8.4 MB instead of 34 GB for max_events = 4096                           */
     uint32_t debug_flags;          /* HOUGH_DEBUG_*: which kernel variant runs where the library would choose by itself.
                                       For tests and measurements; 0 in production.  They change speed, never results.
                                       (The library reads no environment variable and keeps no state outside a context,
@@ -105,9 +110,20 @@ enum {
 /*
  * Create a context.  HOST pointers.  Validates cfg, builds the constant tables in double precision
  * (cos/sin of the phi0 bin centres, d0 bin centres, 2*d0, d0^2, NK/(2*kappa_max)), rounds each once to
- * fp32, uploads them, and allocates the workspaces (prepared hits: 36 B per hit = sorted record 16 B +
- * unsorted record 16 B + sort key 4 B, plus 9 B per hit of staging if host_chunk_events > 0; peak bitmap:
- * 1 bit per bin per event; jet keys: 8 B per stored peak; optional host-path planes).  Synchronous.
+ * fp32, uploads them, and allocates ALL the workspaces: no other call allocates (no hidden
+ * allocations).  Device footprint in bytes, with bins = ND*NPHI*NK, PE = max_plane_events (or max_events if 0),
+ * FE = host_chunk_events (or max_events if 0), CC = max_candidates_per_event (or its default), CC2 = CC rounded up to
+ * a power of two:
+ *     36 * max_hits                                        prepared hits (sorted + unsorted record, sort key)
+ *   + PE * (bins / 8 + 2 * ceil(bins / 256))               peak bitmap and group counts of hough_peaks
+ *   + 8 * max_events * max_peaks_per_event                 clustering keys of hough_jets
+ *   + FE * (16 * CC + 8 * CC2 + 8)                         fused path: candidates, their sort keys, counters
+ *   + tables and per-event segment / bucket tables         (a few KB per event)
+ * and, if host_chunk_events > 0 (hough_trigger_host*):
+ *   + 9 * max_hits + 4 * bins                              staged hits; the planes of ONE event (overflow fallback)
+ *   + max_events * (28 * max_peaks_per_event + 20 * max_jets_per_event + 16 * max_vertices_per_event + 18)
+ *                                                          peak / track / jet / vertex lists and counters of the batch
+ * Synchronous.
  */
 int hough_create(const hough_config* cfg, hough_ctx** out);
 int hough_destroy(hough_ctx* ctx);
@@ -142,7 +158,8 @@ int hough_vote(hough_ctx* ctx, uint32_t n_events, const uint32_t* d_hit_offsets,
  * written in ascending lin.
  *   d_peaks   [n_events][max_peaks_per_event]; only the first min(n_peaks[e], max_peaks) records are written
  *   d_n_peaks [n_events] u32: the TRUE number of peaks found (may exceed the capacity)
- * l_min must be in [1, n_layers].  Precondition: the planes are accumulators as hough_vote writes them, i.e.
+ * l_min must be in [1, n_layers]; n_events <= max_plane_events (if that is not 0) and <= max_events.
+ * Precondition: the planes are accumulators as hough_vote writes them, i.e.
  * count[b] >= popcount(mask[b]) for every bin (a bin with count < l_min is rejected without reading its mask).
  */
 int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, const uint16_t* d_mask,

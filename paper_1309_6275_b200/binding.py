@@ -40,7 +40,8 @@ class HoughConfig(C.Structure):
                 ("max_peaks_per_event", C.c_uint32), ("max_jets_per_event", C.c_uint32),
                 ("host_chunk_events", C.c_uint32), ("max_candidates_per_event", C.c_uint32),
                 ("n_vtx_phi", C.c_uint32), ("n_vtx_r", C.c_uint32), ("vtx_r_min", C.c_float), ("vtx_r_max", C.c_float),
-                ("max_vertices_per_event", C.c_uint32), ("vote_flags", C.c_uint32), ("debug_flags", C.c_uint32)]
+                ("max_vertices_per_event", C.c_uint32), ("vote_flags", C.c_uint32), ("max_plane_events", C.c_uint32),
+                ("debug_flags", C.c_uint32)]
 
 
 class HoughError(RuntimeError):
@@ -146,12 +147,13 @@ class Hough:
                  max_events: int = 1, max_hits: int = 1 << 16, max_peaks_per_event: int = 4096,
                  max_jets_per_event: int = 256, host_chunk_events: int = 0, max_candidates_per_event: int = 0,
                  n_vtx_phi: int = 0, n_vtx_r: int = 0, vtx_r_min: float = 30.0, vtx_r_max: float = 430.0,
-                 max_vertices_per_event: int = 64, vote_flags: int = 0, debug_flags: int = 0):
+                 max_vertices_per_event: int = 64, vote_flags: int = 0, max_plane_events: int = 0,
+                 debug_flags: int = 0):
         self.lib = load_library()
         self.cfg = HoughConfig(n_phi0, n_kappa, n_d0, kappa_max, d0_min, d0_max, b_tesla, n_layers, max_events,
                                max(1, max_hits), max_peaks_per_event, max_jets_per_event, host_chunk_events,
                                max_candidates_per_event, n_vtx_phi, n_vtx_r, vtx_r_min, vtx_r_max,
-                               max_vertices_per_event, vote_flags, debug_flags)
+                               max_vertices_per_event, vote_flags, max_plane_events, debug_flags)
         self._ctx = C.c_void_p()
         _check(self.lib.hough_create(C.byref(self.cfg), C.byref(self._ctx)), "hough_create")
 
@@ -159,7 +161,7 @@ class Hough:
     def for_workload(cls, w, max_events: Optional[int] = None, max_hits: Optional[int] = None,
                      host_chunk_events: int = 0, max_peaks: Optional[int] = None,
                      max_candidates: int = 0, vgrid=None, max_vertices: int = 64, vote_flags: int = 0,
-                     debug_flags: int = 0) -> "Hough":
+                     max_plane_events: int = 0, debug_flags: int = 0) -> "Hough":
         """vgrid: None, or (n_vtx_phi, n_vtx_r, r_min, r_max) for the second Hough transform (hough_vertices)."""
         ne = w.n_events if max_events is None else max_events
         if max_hits is None:
@@ -169,7 +171,7 @@ class Hough:
         return cls(w.n_phi0, w.n_kappa, w.n_d0, w.kappa_max, w.d0_min, w.d0_max, w.b_tesla, w.n_layers, ne,
                    min(mh, 0xFFFFFFFF), w.max_peaks if max_peaks is None else max_peaks, w.max_jets,
                    host_chunk_events, max_candidates, *((0, 0, 30.0, 430.0) if vgrid is None else vgrid), max_vertices, vote_flags,
-                   debug_flags)
+                   max_plane_events, debug_flags)
 
     # -- lifetime ---------------------------------------------------------------------------------
     def close(self):

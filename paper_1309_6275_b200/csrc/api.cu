@@ -81,6 +81,7 @@ bool config_ok(const hough_config* g)
     if (g->max_hits < 1 || g->max_hits > 0xffffffffull) return false;
     if (g->max_peaks_per_event < 1 || g->max_jets_per_event < 1) return false;
     if (g->host_chunk_events > g->max_events) return false;
+    if (g->max_plane_events > g->max_events) return false;
     if (g->max_candidates_per_event > (1u << 24)) return false;
     if (g->vote_flags & ~(uint32_t)(HOUGH_VOTE_HEMI | HOUGH_VOTE_FILL)) return false;
     if (g->debug_flags & ~(uint32_t)(HOUGH_DEBUG_NO_MIRROR | HOUGH_DEBUG_TILES_COUNT | HOUGH_DEBUG_TILES_MASK)) return false;
@@ -215,8 +216,10 @@ int hough_create(const hough_config* cfg, hough_ctx** out)
     if (c->has_mo) A(dev_alloc(&c->d_tilewin_mo, (size_t)c->vote_mo.nk_seg * HOUGH_MAX_LAYERS * c->vote_mo.n_strips));
     A(dev_alloc(&c->d_status, 2));
     A(dev_alloc(&c->d_tilectr, 2));
-    A(dev_alloc(&c->d_bitmap, (size_t)cfg->max_events * (bins / 8)));
-    A(dev_alloc(&c->d_grpcnt, (size_t)cfg->max_events * ((bins + 255) / 256)));
+    // peak-finder scratch of the accumulator path: sized for the events ONE hough_peaks call may bring
+    c->plane_events = cfg->max_plane_events ? cfg->max_plane_events : cfg->max_events;
+    A(dev_alloc(&c->d_bitmap, (size_t)c->plane_events * (bins / 8)));
+    A(dev_alloc(&c->d_grpcnt, (size_t)c->plane_events * ((bins + 255) / 256)));
     A(dev_alloc(&c->d_jetkeys, (size_t)cfg->max_events * cfg->max_peaks_per_event));
     // fused vote -> peaks: candidate buffers for the events of one fused launch
     c->fused_events = cfg->host_chunk_events ? cfg->host_chunk_events : cfg->max_events;
@@ -325,7 +328,7 @@ int hough_peaks(hough_ctx* ctx, uint32_t n_events, const uint16_t* d_count, cons
                 hough_peak* d_peaks, uint32_t* d_n_peaks, void* stream)
 {
     if (!ctx || !d_count || !d_mask || !d_peaks || !d_n_peaks) return HOUGH_EINVAL;
-    if (n_events > ctx->cfg.max_events || l_min < 1 || l_min > ctx->cfg.n_layers) return HOUGH_EINVAL;
+    if (n_events > ctx->plane_events || l_min < 1 || l_min > ctx->cfg.n_layers) return HOUGH_EINVAL;
     if (((uintptr_t)d_count | (uintptr_t)d_mask) & 15u) return HOUGH_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     ctx->last_stream = st;

@@ -77,8 +77,9 @@ struct hough_ctx {
     TileWin* d_tilewin_mo;                    // the same for the mask-tile plan of the fused path (vote_mo), if any
     uint32_t* d_status;                       // [2]: sticky bits, trig-risk counter
     uint32_t* d_tilectr;                      // [2]: vote kernel tile ticket + finished-block count (zero between launches)
-    uint8_t* d_bitmap;                        // [max_events][bins/8], a group's bytes defined where d_grpcnt > 0
-    uint16_t* d_grpcnt;                       // [max_events][ceil(bins/256)] peaks per group of 256 / 512 bins
+    uint32_t plane_events;                    // events per hough_peaks call: cfg.max_plane_events, or max_events if that is 0
+    uint8_t* d_bitmap;                        // [plane_events][bins/8], a group's bytes defined where d_grpcnt > 0
+    uint16_t* d_grpcnt;                       // [plane_events][ceil(bins/256)] peaks per group of 256 / 512 bins
     uint64_t* d_jetkeys;                      // [max_events][max_peaks]
     // fused vote -> peaks
     uint32_t fused_events;                    // events per fused launch the buffers below are sized for

@@ -62,6 +62,7 @@ def test_config_struct_layout_matches_header():
         offsetof(hough_config, max_events), offsetof(hough_config, max_candidates_per_event));
         printf("%zu %zu %zu %zu %zu\n", offsetof(hough_config, vtx_r_min), offsetof(hough_config, max_vertices_per_event), sizeof(hough_vertex),
                offsetof(hough_config, vote_flags), offsetof(hough_config, debug_flags));
+        printf("%zu\n", offsetof(hough_config, max_plane_events));
         return 0; }'''
     exe = "/tmp/hough_layout_probe"
     subprocess.run(["gcc", "-x", "c", "-", "-I", os.path.join(ROOT, "include"), "-o", exe], input=src, text=True, check=True)
@@ -71,7 +72,7 @@ def test_config_struct_layout_matches_header():
     assert vals[6] == B.HoughConfig.max_events.offset and vals[7] == B.HoughConfig.max_candidates_per_event.offset
     assert vals[8] == B.HoughConfig.vtx_r_min.offset and vals[9] == B.HoughConfig.max_vertices_per_event.offset
     assert vals[10] == B.VERTEX_DTYPE.itemsize == 16 and vals[11] == B.HoughConfig.vote_flags.offset
-    assert vals[12] == B.HoughConfig.debug_flags.offset
+    assert vals[12] == B.HoughConfig.debug_flags.offset and vals[13] == B.HoughConfig.max_plane_events.offset
     assert vals[3] == B.PEAK_DTYPE.itemsize == 8 and vals[4] == B.TRACK_DTYPE.itemsize == 20
     assert vals[5] == B.JET_DTYPE.itemsize == 20
 
@@ -118,8 +119,10 @@ def test_library_reads_no_environment_variable_and_rejects_unknown_debug_flags()
     lib = B.load_library()
     ctx = C.c_void_p()
     for flags in (8, B.DEBUG_TILES_COUNT | B.DEBUG_TILES_MASK):
-        bad = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0, flags)
+        bad = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 8, 1, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0, 0, flags)
         assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
+    bad = B.HoughConfig(512, 256, 1, 1.14e-3, 0, 0, 3.8, 8, 4, 100, 16, 16, 0, 0, 0, 0, 0, 0, 0, 0, 5, 0)   # max_plane_events > max_events
+    assert lib.hough_create(C.byref(bad), C.byref(ctx)) == -1
 
 
 def test_product_path_never_touches_the_oracle():
