@@ -168,13 +168,16 @@ def measured_peaks():
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
 
 
-def traffic_from_profiles(kernel_substr: str):
+def traffic_from_profiles(kernel_substr: str, tag: str = ""):
     """(dram__bytes_read.sum + dram__bytes_write.sum in GB per launch, file name, FMA-pipe busy fraction) of the newest
-    committed `ncu --page raw --csv` export under profiles/ whose kernel name contains kernel_substr; (None, None, None)
-    if there is none.  The pipe fraction is sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed / 100: what
+    committed `ncu --page raw --csv` export under profiles/ whose kernel name contains kernel_substr (e.g. "vote_kernel<1,"
+    = the 3D kernels) and whose file name contains `tag` (the workload the capture was taken on); (None, None, None) if
+    there is none.  The pipe fraction is sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_elapsed / 100: what
     the FP32 pipe was measured to do, next to the model-work fraction the roofline reports."""
     best = (None, None, None)
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_ncu_raw.csv"))):
+        if tag and tag not in os.path.basename(path):
+            continue
         try:
             rows = list(csv.reader(open(path, newline="")))
         except Exception:
@@ -450,15 +453,26 @@ def measure_config(name: str, hbm_gbs, sm_max_mhz, peak_src, steps: int = 3):
             d["latency_us"] = 1e3 * ms / reps
         else:
             bins_w = 0 if path == "fused" else w.bins_per_event * w.n_events * reps
+            # a committed capture of this config's fused launch (same events per launch), if there is one
+            tr = traffic_from_profiles("vote_kernel<0," if mode == "2d" else "vote_kernel<1,", "_" + name.lower() + "_") \
+                if path == "fused" else None
             d["roofline"] = vote_roofline(mode, votes * reps, bins_w, stage[1], n_launch, hbm_gbs, sm_max_mhz, peak_src,
                                           "vote_kernel<fused>" if path == "fused" else "vote_kernel",
-                                          tile_kind=run.tile_kind)
+                                          traffic=tr if tr and tr[0] is not None else None, tile_kind=run.tile_kind)
             if path == "planes":
                 d["roofline_stencil"] = stencil_roofline(w.bins_per_event * w.n_events * reps, stage[2], n_launch, hbm_gbs)
         res[path] = d
         run.close()
         torch.cuda.empty_cache()
     return res
+
+
+def p4_traffic(n_tracks: int, path: str, n_events: int):
+    """The committed capture of the P4 fused launch with this many tracks per event (32 events per launch), if any."""
+    if path != "fused" or n_events != 32:
+        return None
+    tr = traffic_from_profiles("vote_kernel<0,", f"_p4x{n_tracks}_")
+    return tr if tr[0] is not None else None
 
 
 def run_p4(args):
@@ -491,7 +505,7 @@ def run_p4(args):
                        "roofline": vote_roofline("2d", votes * args.steps, 0 if path == "fused" else w.bins_per_event * E * args.steps,
                                                  stage[1], args.steps, hbm_gbs, sm_max_mhz, peak_src,
                                                  "vote_kernel<fused>" if path == "fused" else "vote_kernel",
-                                                 tile_kind=run.tile_kind)}
+                                                 traffic=p4_traffic(n, path, E), tile_kind=run.tile_kind)}
             if path == "fused":
                 d["peaks_per_event"] = float(run.out["n_peaks"].float().mean().item())
                 last = (w, batch, ms, stage, launches, votes)
@@ -800,7 +814,7 @@ def run_ours(args):
     votes_timed = votes_per_step * args.steps
     fused = args.path == "fused"
     kern = "vote_kernel<fused>" if fused else "vote_kernel"
-    traffic = traffic_from_profiles("vote_kernel") if (w.name == "C5" and chunk == 128) else None
+    traffic = traffic_from_profiles("vote_kernel<1,") if (w.name == "C5" and chunk == 128) else None
     roofline = vote_roofline(mode, votes_timed, 0 if fused else bins * E * args.steps, stage[1], n_launch, hbm_gbs,
                              sm_max_mhz, peak_src, kern, traffic, tile_kind=main_tile_kind)
 
